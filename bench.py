@@ -1,0 +1,332 @@
+#!/usr/bin/env python
+"""Device-timed benchmark of the B200 Joseph cone-beam forward projector (libfp.so).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config C3] [--impl ours|reference]
+
+One "step" is one pass of the whole hot path (geometry ingest, ray set-up, layout stage if the
+pose needs it, sampling loop, weight + store) over one batch of synthetic
+input: the full orbit of the configuration (C3: 360 projections of a 512^3 volume onto 768^2).
+Prints ONE JSON line (rank 0).  DESIGN.md "Measurement" states how every number is formed.
+
+The oracle (oracle/) is used only by the cpu_baseline leg and by --impl reference.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import tempfile
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "512^3 cone-beam projections/s"
+UNIT = "projections/s"
+TAP_BYTES = 16           # 4 taps x 4 B per sample: the paper's "memory access rate"
+FALLBACK_HBM_GBS = 6650.0
+
+
+def measured_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        try:
+            return json.load(open(p)), "measured"
+        except Exception:
+            pass
+    return {"hbm_gbs": FALLBACK_HBM_GBS}, "fallback"
+
+
+class ClockSampler:
+    """nvidia-smi clocks and throttle reasons DURING the timed region (B200_PROFILING.md)."""
+
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,"
+         "clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index: int):
+        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        self.p = None
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", "-i", str(gpu_index), "--query-gpu=" + self.Q,
+                                       "--format=csv,noheader,nounits", "-lms", "100"],
+                                      stdout=self.f, stderr=subprocess.DEVNULL)
+        except Exception:
+            self.p = None
+
+    def stop(self):
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        if self.p is None:
+            return out
+        self.p.terminate()
+        try:
+            self.p.wait(timeout=5)
+        except Exception:
+            self.p.kill()
+        self.f.flush()
+        self.f.seek(0)
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for line in self.f.read().splitlines():
+            c = [x.strip() for x in line.split(",")]
+            if len(c) < 9:
+                continue
+            try:
+                sm.append(float(c[1]))
+                mx.append(float(c[2]))
+            except ValueError:
+                continue
+            for n, v in zip(names, c[5:9]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        self.f.close()
+        try:
+            os.unlink(self.f.name)
+        except OSError:
+            pass
+        if sm:
+            out.update(sm_mhz=statistics.median(sm), sm_max_mhz=max(mx), samples=len(sm))
+        out["reasons"] = sorted(reasons)
+        return out
+
+
+def oracle_sample(cfg, geom, vol_np, max_seconds=20.0):
+    """Time the oracle, as it stands, on a bounded sample of the workload: whole detector rows of
+    projection 0 and of the projection at 1/8 of the orbit (both driving axes for circular
+    orbits), using every host core.  Returns (projections/s, samples/s, cores, description,
+    ids, values, mfl, pathlen, margins)."""
+    import oracle
+    cores = oracle.host_cores()
+    projs = [0, cfg.n_proj // 8]
+    # calibrate on a few rows, then size the sample for ~max_seconds of wall time
+    rows_cal = max(1, min(cfg.nv, 4))
+    def ids_for(rows):
+        vs = np.linspace(0, cfg.nv - 1, rows).round().astype(np.int32)
+        p, v, u = np.meshgrid(np.array(projs, dtype=np.int32), vs, np.arange(cfg.nu, dtype=np.int32), indexing="ij")
+        return np.stack([p.ravel(), v.ravel(), u.ravel()], axis=1).astype(np.int32)
+    ids = ids_for(rows_cal)
+    t0 = time.perf_counter()
+    oracle.project_rays(vol_np, cfg.voxel_size, cfg.origin, geom, ids, threads=cores)
+    t_cal = time.perf_counter() - t0
+    rows = int(max(rows_cal, min(cfg.nv, rows_cal * max_seconds / max(t_cal, 1e-3))))
+    ids = ids_for(rows)
+    t0 = time.perf_counter()
+    val, mfl, pl, mg = oracle.project_rays(vol_np, cfg.voxel_size, cfg.origin, geom, ids, threads=cores)
+    dt = time.perf_counter() - t0
+    n_samples = int(np.maximum(mfl[:, 2] - mfl[:, 1] + 1, 0).sum())
+    rays_per_proj = cfg.nu * cfg.nv
+    proj_per_s = (len(ids) / rays_per_proj) / dt
+    desc = "%d of %d detector rows (all %d columns) of projections %s: %d rays, %d samples in %.1f s" % (
+        rows, cfg.nv, cfg.nu, projs, len(ids), n_samples, dt)
+    return proj_per_s, n_samples / dt, cores, desc, ids, val, mfl, pl, mg
+
+
+def run_reference(args):
+    """--impl reference: the fp64 CPU oracle as the reference arm (there is no reference code)."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    from paper_1609_00958_b200 import synth
+    cfg = synth.CONFIGS[args.config]
+    geom = synth.make_geometry(cfg)
+    vol = synth.make_volume(cfg, device="cpu").numpy()
+    budget = 60.0 / max(1, args.steps + args.warmup)
+    vals = []
+    desc, cores = "", 0
+    for k in range(args.warmup + args.steps):
+        pps, sps, cores, desc, *_ = oracle_sample(cfg, geom, vol, max_seconds=min(20.0, budget))
+        if k >= args.warmup:
+            vals.append((pps, sps))
+    pps = statistics.median(v[0] for v in vals)
+    sps = statistics.median(v[1] for v in vals)
+    line = {
+        "impl": "reference", "metric": METRIC, "value": pps, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * cfg.n_proj / pps,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": workload_name(cfg), "extrapolated": True},
+        "gsamples_per_s": sps / 1e9,
+        "cpu_baseline": {"value": pps, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc},
+        "e2e": {"value": pps, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+    }
+    print(json.dumps(line))
+    return 0
+
+
+def workload_name(cfg):
+    return "%s: %dx%dx%d fp32 volume, %d projections (%s orbit) onto %dx%d" % (
+        cfg.name, *cfg.n, cfg.n_proj, cfg.orbit, cfg.nu, cfg.nv)
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", default="C3", choices=["C1", "C2", "C3", "C4", "C5"])
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--kernel", type=int, default=0, help="FP_OPT_KERNEL value (0 = auto)")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 0)
+    if args.impl == "reference":
+        return run_reference(args)
+
+    import torch
+    from paper_1609_00958_b200 import fp, synth
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: there is no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    fp.load()
+
+    cfg = synth.CONFIGS[args.config]
+    geom = synth.make_geometry(cfg)
+    vol = synth.make_volume(cfg, device="cuda")
+    batch = cfg.batch or cfg.n_proj
+    out = torch.empty((cfg.n_proj, cfg.nv, cfg.nu), device="cuda", dtype=torch.float32)
+    P = fp.Projector(*cfg.n, cfg.voxel_size, cfg.origin)
+    if args.kernel:
+        P.set_option(fp.OPT_KERNEL, args.kernel)
+    stream = torch.cuda.current_stream()
+
+    def step():
+        launches, samples = 0, None
+        for p0 in range(0, cfg.n_proj, batch):
+            p1 = min(cfg.n_proj, p0 + batch)
+            P.project(vol, geom[p0:p1], cfg.nu, cfg.nv, out=out[p0:p1], stream=stream)
+            launches += P.last_launch_count()
+        return launches
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+
+    for _ in range(args.warmup):
+        step()
+    torch.cuda.synchronize()
+    # sample count of one step (outside the timed region: fp_last_sample_count synchronises)
+    samples = 0
+    for p0 in range(0, cfg.n_proj, batch):
+        p1 = min(cfg.n_proj, p0 + batch)
+        P.project(vol, geom[p0:p1], cfg.nu, cfg.nv, out=out[p0:p1], stream=stream)
+        samples += P.last_sample_count()
+
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps + 1)]
+    barrier()
+    torch.cuda.synchronize()
+    clocks = ClockSampler(local_rank)
+    time.sleep(0.25)
+    launches = 0
+    ev[0].record(stream)
+    for k in range(args.steps):
+        launches += step()
+        ev[k + 1].record(stream)
+    torch.cuda.synchronize()
+    barrier()
+    clk = clocks.stop()
+    step_ms = [ev[k].elapsed_time(ev[k + 1]) for k in range(args.steps)]
+    total_ms = ev[0].elapsed_time(ev[args.steps])
+    t = torch.tensor([total_ms], device="cuda", dtype=torch.float64)
+    if dist is not None:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    total_ms = float(t.item())
+    ms_per_step = total_ms / args.steps
+    proj_per_s = world * cfg.n_proj / (ms_per_step * 1e-3)
+    samples_per_s = world * samples / (ms_per_step * 1e-3)
+
+    # ---- end to end through fp_project_host: pinned host volume in, pinned host projections out
+    e2e = None
+    if not args.no_e2e:
+        vol_h = vol.cpu().pin_memory()
+        out_h = torch.empty((cfg.n_proj, cfg.nv, cfg.nu), dtype=torch.float32).pin_memory()
+        P2 = fp.Projector(*cfg.n, cfg.voxel_size, cfg.origin)
+        P2.project_host(vol_h, geom, cfg.nu, cfg.nv, out_host=out_h)          # warm-up (allocations)
+        n_e2e = max(1, min(args.steps, 3))
+        barrier()
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        for _ in range(n_e2e):
+            P2.project_host(vol_h, geom, cfg.nu, cfg.nv, out_host=out_h)      # synchronises before returning
+        dt = time.perf_counter() - t0
+        t = torch.tensor([dt], device="cuda", dtype=torch.float64)
+        if dist is not None:
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        dt = float(t.item())
+        e2e = {"value": world * cfg.n_proj * n_e2e / dt, "unit": UNIT,
+               "h2d_bytes_per_step": int(vol_h.numel() * 4 + geom.size * 8),
+               "d2h_bytes_per_step": int(out_h.numel() * 4), "steps": n_e2e,
+               "same_result_as_device_path": bool(torch.equal(out_h, out.cpu()))}
+        P2.close()
+        del vol_h
+
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return 0
+
+    peaks, peak_kind = measured_peaks()
+    vol_bytes = vol.numel() * 4
+    out_bytes_per_proj = cfg.nu * cfg.nv * 4
+    # algorithmic HBM bytes per projection: the volume once + the projection written once
+    algo_bytes_per_step = cfg.n_proj * (vol_bytes + out_bytes_per_proj)
+    kernel_ms = ms_per_step            # one sampling launch per fp_project; the step is that launch
+    achieved = algo_bytes_per_step / (kernel_ms * 1e-3) / 1e9
+    roofline = {"bound": "hbm", "achieved": achieved, "peak": peaks["hbm_gbs"], "unit": "GB/s",
+                "frac": achieved / peaks["hbm_gbs"], "traffic": None, "peak_kind": peak_kind,
+                "kernel": "fp_direct_kernel", "algorithmic_bytes_per_launch": algo_bytes_per_step // max(1, (cfg.n_proj + batch - 1) // batch)}
+
+    cpu_baseline = None
+    parity = None
+    if not args.no_cpu_baseline and world == 1:
+        vol_np = vol.cpu().numpy()
+        pps, sps, cores, desc, ids, val, mfl, pl, mg = oracle_sample(cfg, geom, vol_np, max_seconds=15.0)
+        cpu_baseline = {"value": pps, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc,
+                        "gsamples_per_s": sps / 1e9, "extrapolated_from_sample": True}
+        g = out[torch.from_numpy(ids[:, 0].astype(np.int64)).cuda(), torch.from_numpy(ids[:, 1].astype(np.int64)).cuda(),
+                torch.from_numpy(ids[:, 2].astype(np.int64)).cuda()].cpu().numpy().astype(np.float64)
+        tol = 2e-5 * np.abs(val) + 1e-6 * pl * float(vol.abs().max().item())
+        parity = {"rays": int(len(ids)), "worst_err_over_tol": float(np.max(np.abs(g - val) / np.maximum(tol, 1e-300)))}
+
+    line = {
+        "metric": METRIC, "value": proj_per_s, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "config": {"workload": workload_name(cfg), "projections_per_call": batch, "replicas": world,
+                   "l2_policy": "inputs larger than L2 (volume %d MB, output %d MB per step; L2 126 MB)" % (
+                       vol_bytes >> 20, (cfg.n_proj * out_bytes_per_proj) >> 20),
+                   "layout_stage_in_timed_region": True},
+        "gsamples_per_s": samples_per_s / 1e9,
+        "samples_per_step": samples,
+        "tap_access_rate_gbs": TAP_BYTES * samples_per_s / 1e9,
+        "step_ms": step_ms,
+        "clocks": clk,
+        "gpu_launches": launches,
+        "e2e": e2e,
+        "roofline": roofline,
+        "cpu_baseline": cpu_baseline,
+        "parity_check": parity,
+        "paper_context": "GTX 970: 176 projections/s (GJP_lin, global memory), 292 GB/s tap access rate, "
+                         "512^3 -> 512^2, 1.04e8 samples/projection (PAPER.md:331 Table 1)",
+    }
+    print(json.dumps(line))
+    if dist is not None:
+        dist.destroy_process_group()
+    return 0
+
+
+if __name__ == "__main__":
+    sys.exit(main())

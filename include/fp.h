@@ -1,0 +1,154 @@
+/*
+ * fp.h -- C ABI of libfp.so: the B200 (sm_100a) Generalized Joseph forward projector.
+ *
+ * The operation is the linear-kernel "Generalized Joseph Projector" (GJP_lin) of
+ * arXiv 1609.00958 (J. Dittmann).  Citations are /root/reference/PAPER.md line numbers with
+ * the section / equation / algorithm they fall in; "reading #k" refers to the table
+ * "Readings of the paper" in DESIGN.md.
+ *
+ * For every detector pixel the library forms the ray r = d - s from the source s to the
+ * pixel centre d (sec. 2.1 Eq. 1), picks the driving axis m = argmax_a |r_a|
+ * (:81 Eq. 2), steps once per voxel slice along m with the increment r~ = r / r_m (:92 Eq. 4,
+ * :104 Eq. 6), interpolates the volume bilinearly in the two transverse axes at the ray's
+ * intersection with each slice plane (:165 Eq. 15, :150 Eq. 13, :142 Eq. 11) and returns
+ *
+ *     out(ray) = voxel_size * ||r~||_2 * sum_{i = i_first}^{i_last} sample(i)      (:211, Alg. 1 :217-269)
+ *
+ * where [i_first, i_last] is the exact set of slices whose intersection point lies in the
+ * zero-padded transverse extent -1 < p_t < N_t (:213 sec. 2.6 "entry and exit points are
+ * calculated exactly"; reading #2).
+ *
+ * Conventions (all entry points):
+ *   - Coordinates: world units.  Voxel (ix, iy, iz) has its CENTRE at
+ *     origin + voxel_size * (ix, iy, iz).  Grid coordinate g = (world - origin) / voxel_size
+ *     (PAPER.md:57 Fig. 1, :63: units normalised to the grid spacing; reading #1).
+ *   - Volume: fp32, C order [nx][ny][nz], z FASTEST (PAPER.md:294 sec. 2.8, :312: the rotation
+ *     axis is parallel to the fastest index).  DEVICE pointer unless the name says _host.
+ *   - Geometry: HOST pointer to n_proj rows of 12 doubles
+ *         { source xyz, det_origin xyz, u-pitch vector xyz, v-pitch vector xyz },
+ *     the centre of pixel (iu, iv) is det_origin + iu * u + iv * v.  The rows are read during
+ *     the call; the caller may reuse the buffer as soon as the call returns.
+ *   - Output: fp32, [n_proj][nv][nu], u fastest (reading #14).  Rays that miss the volume
+ *     (and the degenerate ray r = 0) write +0.0f.
+ *   - Streams: every kernel and copy is enqueued on the given stream; fp_project does not
+ *     synchronise the host with the device.  Outputs are valid once the stream reaches that point.
+ *   - Ownership: the caller owns the volume, the geometry and the outputs.  The library owns
+ *     the context, its internal volume copies and workspaces (freed by fp_destroy).
+ *   - Errors: status codes only, nothing is thrown.  fp_last_error(ctx) holds the text of the
+ *     most recent failure on that context.  A context is not thread-safe; different contexts
+ *     are independent.  Non-finite geometry gives unspecified output values but never a fault.
+ *   - There is NO CPU fallback: without a CUDA device every compute entry point returns
+ *     FP_ERR_CUDA.
+ */
+#ifndef FP_H_
+#define FP_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct fp_ctx fp_ctx;                 /* opaque, library-owned */
+typedef struct CUstream_st *fp_stream;        /* a cudaStream_t (0 = the legacy default stream) */
+
+typedef enum {
+    FP_OK = 0,
+    FP_ERR_INVALID_ARG = 1,
+    FP_ERR_CUDA = 2,
+    FP_ERR_OOM = 3,
+    FP_ERR_UNSUPPORTED = 4
+} fp_status;
+
+/* fp_set_option keys.  Options are explicit; no environment variable changes behaviour. */
+enum {
+    /* Sampling-kernel variant: FP_KERNEL_AUTO picks per projection. */
+    FP_OPT_KERNEL = 1,
+    /* 1 (default): the volume contents may have changed since the last call, internal copies
+     * are rebuilt by every fp_project that needs them.  0: internal copies made by fp_prepare
+     * (or the first fp_project) stay valid until the next fp_prepare. */
+    FP_OPT_VOLATILE = 2,
+    /* Interpolation kernel w(d): FP_INTERP_LINEAR (Eq. 13) or
+     * FP_INTERP_SPLINE (:152 Eq. 14). */
+    FP_OPT_INTERP = 3,
+    /* 1 (default): a y-fastest permuted copy of the volume is built when a projection has
+     * z-driven rays, so that their in-plane taps are contiguous (sec. 2.8).
+     * 0: z-driven rays read the caller's layout with strided taps. */
+    FP_OPT_PERMUTED_COPY = 4,
+    /* 1: fp_project accumulates the number of samples sum(i_last - i_first + 1) for
+     * fp_last_sample_count (default 1; one atomic per thread block). */
+    FP_OPT_COUNT_SAMPLES = 5
+};
+
+enum { FP_KERNEL_AUTO = 0, FP_KERNEL_DIRECT = 1, FP_KERNEL_STAGED = 2 };
+enum { FP_INTERP_LINEAR = 0, FP_INTERP_SPLINE = 1 };
+
+/*
+ * fp_create: describe the voxel grid (PAPER.md:57 Fig. 1, :63 sec. 2).
+ *   nx, ny, nz  >= 1, nx*ny*nz < 2^40;   voxel_size > 0 and finite;
+ *   origin[3]   host pointer, world position of the centre of voxel (0,0,0), finite.
+ * Allocates nothing on the device.  Returns FP_ERR_INVALID_ARG on bad arguments.
+ */
+fp_status fp_create(int nx, int ny, int nz, double voxel_size, const double origin[3], fp_ctx **out);
+
+/* fp_destroy: frees the context and every device allocation it owns (synchronises the device). */
+fp_status fp_destroy(fp_ctx *ctx);
+
+fp_status fp_set_option(fp_ctx *ctx, int key, int value);
+fp_status fp_get_option(fp_ctx *ctx, int key, int *value);
+
+/*
+ * fp_prepare: volume-layout stage (sec. 2.8) run now, on `stream`: builds the
+ * internal copies of vol_dev that the configured kernels want.  Optional: fp_project runs
+ * the stage itself when it needs a copy that is missing or (FP_OPT_VOLATILE = 1) stale.
+ */
+fp_status fp_prepare(fp_ctx *ctx, const float *vol_dev, fp_stream stream);
+
+/*
+ * fp_project: the forward projection (Alg. 1) of n_proj poses.
+ *   vol_dev    device, fp32 [nx][ny][nz]
+ *   n_proj     >= 0 (0 is a no-op)
+ *   geom_host  host, double [n_proj][12]
+ *   nu, nv     >= 1 detector pixels along u and v
+ *   out_dev    device, fp32 [n_proj][nv][nu], fully overwritten
+ */
+fp_status fp_project(fp_ctx *ctx, const float *vol_dev, int n_proj, const double *geom_host,
+                     int nu, int nv, float *out_dev, fp_stream stream);
+
+/*
+ * fp_project_host: the same with HOST volume and HOST output; the library copies the volume to
+ * the device, projects in batches and copies the result back.  Synchronises before returning.
+ * This is the end-to-end entry point (bench.py "e2e").
+ *   vol_host   host, fp32 [nx][ny][nz]     out_host   host, fp32 [n_proj][nv][nu]
+ */
+fp_status fp_project_host(fp_ctx *ctx, const float *vol_host, int n_proj, const double *geom_host,
+                          int nu, int nv, float *out_host);
+
+/*
+ * fp_ray_ranges: per-ray set-up only (PAPER.md:71-106 Eqs. 1-6, Alg. 1 l.1-5, :213): writes
+ * { m, i_first, i_last } per pixel; a miss is { m, 0, -1 }, the degenerate ray { 0, 0, -1 }.
+ * The decisions are taken in IEEE fp64 in the operation order DESIGN.md fixes, so they are
+ * bit-identical to the oracle's.
+ *   mfl_dev    device, int32 [n_proj][nv][nu][3]
+ */
+fp_status fp_ray_ranges(fp_ctx *ctx, int n_proj, const double *geom_host, int nu, int nv,
+                        int32_t *mfl_dev, fp_stream stream);
+
+/*
+ * fp_last_sample_count: number of samples (visited slices summed over rays) of the most recent
+ * fp_project / fp_project_host on this context; synchronises the stream that call used.
+ * This is the unit of the paper's "memory access rate" = 16 B x samples / time.
+ */
+fp_status fp_last_sample_count(fp_ctx *ctx, unsigned long long *n);
+
+/* fp_last_launch_count: how many kernels of this library the most recent fp_project enqueued. */
+fp_status fp_last_launch_count(fp_ctx *ctx, int *n);
+
+const char *fp_status_string(fp_status s);
+const char *fp_last_error(fp_ctx *ctx);
+const char *fp_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* FP_H_ */

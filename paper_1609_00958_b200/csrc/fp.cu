@@ -1,0 +1,450 @@
+// fp.cu -- host side of libfp.so: the C ABI declared in include/fp.h.
+// Argument validation, per-projection planning on the host, workspace ownership, launches.
+// No arithmetic of the method lives here except the host planning heuristics (which kernel,
+// which warp orientation); every step of the hot path runs in the kernels of fp_kernels.cuh.
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include <cuda_runtime.h>
+
+#include "../../include/fp.h"
+#include "fp_kernels.cuh"
+
+using namespace fpk;
+
+struct fp_ctx {
+    GridDesc G;
+    // options
+    int opt_kernel = FP_KERNEL_AUTO;
+    int opt_volatile = 1;
+    int opt_interp = FP_INTERP_LINEAR;
+    int opt_permuted = 1;
+    int opt_count = 1;
+    // layout stage: y-fastest copy [nz][nx][ny] for z-driven rays
+    float *vol_perm = nullptr;
+    const float *perm_src = nullptr;
+    bool perm_valid = false;
+    // per-call workspaces
+    ProjDesc *proj_dev = nullptr;
+    int proj_cap = 0;
+    unsigned long long *count_dev = nullptr;
+    cudaStream_t last_stream = nullptr;
+    bool counted = false;
+    int last_launches = 0;
+    // fp_project_host workspaces
+    float *hvol_dev = nullptr;
+    float *hout_dev[2] = {nullptr, nullptr};
+    size_t hout_cap = 0;
+    cudaStream_t hstream[2] = {nullptr, nullptr};
+    cudaEvent_t hevent[2] = {nullptr, nullptr};
+    std::string err;
+};
+
+static fp_status fail(fp_ctx *c, fp_status s, const std::string &msg)
+{
+    if (c) c->err = msg;
+    return s;
+}
+
+static fp_status cuda_fail(fp_ctx *c, cudaError_t e, const char *what)
+{
+    char buf[512];
+    snprintf(buf, sizeof buf, "%s: %s (%s)", what, cudaGetErrorString(e), cudaGetErrorName(e));
+    cudaGetLastError();   // clear the sticky flag of non-fatal errors
+    return fail(c, e == cudaErrorMemoryAllocation ? FP_ERR_OOM : FP_ERR_CUDA, buf);
+}
+
+#define FP_CUDA(ctx, call)                                             \
+    do {                                                               \
+        cudaError_t e_ = (call);                                       \
+        if (e_ != cudaSuccess) return cuda_fail((ctx), e_, #call);     \
+    } while (0)
+
+static size_t n_voxels(const fp_ctx *c) { return (size_t)c->G.n[0] * c->G.n[1] * c->G.n[2]; }
+
+extern "C" const char *fp_version(void) { return "libfp 0.1 (sm_100a)"; }
+
+extern "C" const char *fp_status_string(fp_status s)
+{
+    switch (s) {
+    case FP_OK: return "FP_OK";
+    case FP_ERR_INVALID_ARG: return "FP_ERR_INVALID_ARG";
+    case FP_ERR_CUDA: return "FP_ERR_CUDA";
+    case FP_ERR_OOM: return "FP_ERR_OOM";
+    case FP_ERR_UNSUPPORTED: return "FP_ERR_UNSUPPORTED";
+    }
+    return "FP_ERR_?";
+}
+
+extern "C" const char *fp_last_error(fp_ctx *ctx) { return ctx ? ctx->err.c_str() : "null context"; }
+
+extern "C" fp_status fp_create(int nx, int ny, int nz, double voxel_size, const double origin[3], fp_ctx **out)
+{
+    if (!out) return FP_ERR_INVALID_ARG;
+    *out = nullptr;
+    if (nx < 1 || ny < 1 || nz < 1 || !origin) return FP_ERR_INVALID_ARG;
+    if (!(voxel_size > 0.0) || !std::isfinite(voxel_size)) return FP_ERR_INVALID_ARG;
+    for (int a = 0; a < 3; ++a)
+        if (!std::isfinite(origin[a])) return FP_ERR_INVALID_ARG;
+    if ((double)nx * ny * nz >= 1099511627776.0) return FP_ERR_INVALID_ARG;
+    fp_ctx *c = new (std::nothrow) fp_ctx;
+    if (!c) return FP_ERR_OOM;
+    c->G.n[0] = nx;
+    c->G.n[1] = ny;
+    c->G.n[2] = nz;
+    c->G.pad_ = 0;
+    c->G.delta = voxel_size;
+    for (int a = 0; a < 3; ++a) c->G.origin[a] = origin[a];
+    *out = c;
+    return FP_OK;
+}
+
+extern "C" fp_status fp_destroy(fp_ctx *c)
+{
+    if (!c) return FP_ERR_INVALID_ARG;
+    cudaDeviceSynchronize();
+    cudaFree(c->vol_perm);
+    cudaFree(c->proj_dev);
+    cudaFree(c->count_dev);
+    cudaFree(c->hvol_dev);
+    for (int k = 0; k < 2; ++k) {
+        cudaFree(c->hout_dev[k]);
+        if (c->hstream[k]) cudaStreamDestroy(c->hstream[k]);
+        if (c->hevent[k]) cudaEventDestroy(c->hevent[k]);
+    }
+    cudaGetLastError();
+    delete c;
+    return FP_OK;
+}
+
+extern "C" fp_status fp_set_option(fp_ctx *c, int key, int value)
+{
+    if (!c) return FP_ERR_INVALID_ARG;
+    switch (key) {
+    case FP_OPT_KERNEL:
+        if (value < FP_KERNEL_AUTO || value > FP_KERNEL_STAGED) return fail(c, FP_ERR_INVALID_ARG, "bad kernel variant");
+        if (value == FP_KERNEL_STAGED) return fail(c, FP_ERR_UNSUPPORTED, "staged kernel not built yet");
+        c->opt_kernel = value;
+        return FP_OK;
+    case FP_OPT_VOLATILE: c->opt_volatile = value != 0; return FP_OK;
+    case FP_OPT_INTERP:
+        if (value != FP_INTERP_LINEAR && value != FP_INTERP_SPLINE) return fail(c, FP_ERR_INVALID_ARG, "bad interpolation kernel");
+        c->opt_interp = value;
+        return FP_OK;
+    case FP_OPT_PERMUTED_COPY:
+        c->opt_permuted = value != 0;
+        c->perm_valid = false;
+        return FP_OK;
+    case FP_OPT_COUNT_SAMPLES: c->opt_count = value != 0; return FP_OK;
+    }
+    return fail(c, FP_ERR_INVALID_ARG, "unknown option key");
+}
+
+extern "C" fp_status fp_get_option(fp_ctx *c, int key, int *value)
+{
+    if (!c || !value) return FP_ERR_INVALID_ARG;
+    switch (key) {
+    case FP_OPT_KERNEL: *value = c->opt_kernel; return FP_OK;
+    case FP_OPT_VOLATILE: *value = c->opt_volatile; return FP_OK;
+    case FP_OPT_INTERP: *value = c->opt_interp; return FP_OK;
+    case FP_OPT_PERMUTED_COPY: *value = c->opt_permuted; return FP_OK;
+    case FP_OPT_COUNT_SAMPLES: *value = c->opt_count; return FP_OK;
+    }
+    return fail(c, FP_ERR_INVALID_ARG, "unknown option key");
+}
+
+// ---------------------------------------------------------------------------- host planning
+
+// Does the open detector rectangle contain directions whose largest component is z?  The ray
+// direction is affine in (iu, iv), so { r : |r_z| > |r_x|, |r_z| > |r_y| } cuts the detector
+// plane in two convex polygons (one per sign of r_z): clip the rectangle against the four half
+// planes of each.  Conservative (closed half planes); only decides whether the permuted copy
+// is worth building -- the kernels are correct either way.
+static bool has_z_driven(const double *g, int nu, int nv)
+{
+    const double c0[3] = {g[3] - g[0], g[4] - g[1], g[5] - g[2]};   // r at (0,0)
+    for (int sign = -1; sign <= 1; sign += 2) {
+        // polygon in (iu, iv)
+        std::vector<std::pair<double, double>> poly = {
+            {-0.5, -0.5}, {nu - 0.5, -0.5}, {nu - 0.5, nv - 0.5}, {-0.5, nv - 0.5}};
+        for (int k = 0; k < 4 && !poly.empty(); ++k) {
+            const int ax = k >> 1;                       // x or y
+            const double sg = (k & 1) ? 1.0 : -1.0;      // sign*r_z -/+ r_ax >= 0
+            const double A = sign * c0[2] + sg * c0[ax];
+            const double B = sign * g[6 + 2] + sg * g[6 + ax];
+            const double C = sign * g[9 + 2] + sg * g[9 + ax];
+            std::vector<std::pair<double, double>> nxt;
+            const size_t n = poly.size();
+            for (size_t q = 0; q < n; ++q) {
+                const auto &a = poly[q], &b = poly[(q + 1) % n];
+                const double fa = A + B * a.first + C * a.second, fb = A + B * b.first + C * b.second;
+                if (fa >= 0) nxt.push_back(a);
+                if ((fa >= 0) != (fb >= 0)) {
+                    const double t = fa / (fa - fb);
+                    nxt.push_back({a.first + t * (b.first - a.first), a.second + t * (b.second - a.second)});
+                }
+            }
+            poly.swap(nxt);
+        }
+        if (poly.size() >= 3) {
+            double area = 0;
+            for (size_t q = 0; q < poly.size(); ++q) {
+                const auto &a = poly[q], &b = poly[(q + 1) % poly.size()];
+                area += a.first * b.second - a.second * b.first;
+            }
+            if (std::fabs(area) > 1e-9) return true;
+        }
+    }
+    return false;
+}
+
+// Warp orientation: lanes run along the detector vector with the larger component along the
+// axis that is contiguous for the central ray's driving axis (adjacent rays
+// should read consecutive addresses).
+static int plan_lane_v(const double *g, int nu, int nv, bool permuted)
+{
+    double r[3];
+    for (int a = 0; a < 3; ++a)
+        r[a] = g[3 + a] + 0.5 * (nu - 1) * g[6 + a] + 0.5 * (nv - 1) * g[9 + a] - g[a];
+    int m = 0;
+    if (std::fabs(r[1]) > std::fabs(r[m])) m = 1;
+    if (std::fabs(r[2]) > std::fabs(r[m])) m = 2;
+    const int fast = (m == 2 && permuted) ? 1 : 2;
+    if (m == 2 && !permuted) return std::fabs(g[9 + 1]) > std::fabs(g[6 + 1]);
+    return std::fabs(g[9 + fast]) > std::fabs(g[6 + fast]);
+}
+
+static fp_status ensure_proj(fp_ctx *c, int n_proj)
+{
+    if (n_proj <= c->proj_cap) return FP_OK;
+    if (c->proj_dev) {
+        // an earlier call may still be reading the old buffer
+        FP_CUDA(c, cudaDeviceSynchronize());
+        cudaFree(c->proj_dev);
+        c->proj_dev = nullptr;
+        c->proj_cap = 0;
+    }
+    const int cap = n_proj + 64;
+    FP_CUDA(c, cudaMalloc(&c->proj_dev, sizeof(ProjDesc) * (size_t)cap));
+    c->proj_cap = cap;
+    return FP_OK;
+}
+
+static fp_status upload_geometry(fp_ctx *c, int n_proj, const double *geom, int nu, int nv, bool permuted,
+                                 cudaStream_t st)
+{
+    fp_status s = ensure_proj(c, n_proj);
+    if (s != FP_OK) return s;
+    std::vector<ProjDesc> h((size_t)n_proj);
+    for (int p = 0; p < n_proj; ++p) {
+        memcpy(h[p].g, geom + 12 * (size_t)p, sizeof(double) * 12);
+        h[p].lane_v = plan_lane_v(h[p].g, nu, nv, permuted);
+        h[p].pad_ = 0;
+    }
+    // pageable source: the runtime stages the bytes before returning, so `h` may die here
+    FP_CUDA(c, cudaMemcpyAsync(c->proj_dev, h.data(), sizeof(ProjDesc) * (size_t)n_proj, cudaMemcpyHostToDevice, st));
+    return FP_OK;
+}
+
+static fp_status build_permuted(fp_ctx *c, const float *vol_dev, cudaStream_t st)
+{
+    const size_t nvox = n_voxels(c);
+    if (!c->vol_perm) FP_CUDA(c, cudaMalloc(&c->vol_perm, nvox * sizeof(float)));
+    const long long R = (long long)c->G.n[0] * c->G.n[1], C = c->G.n[2];
+    dim3 grid((unsigned)((R + 31) / 32), (unsigned)((C + 31) / 32));
+    fp_transpose_kernel<<<grid, 256, 0, st>>>(vol_dev, c->vol_perm, R, C);
+    FP_CUDA(c, cudaGetLastError());
+    c->perm_src = vol_dev;
+    c->perm_valid = true;
+    c->last_launches += 1;
+    return FP_OK;
+}
+
+extern "C" fp_status fp_prepare(fp_ctx *c, const float *vol_dev, fp_stream stream)
+{
+    if (!c || !vol_dev) return fail(c, FP_ERR_INVALID_ARG, "fp_prepare: null argument");
+    c->last_launches = 0;
+    if (!c->opt_permuted) return FP_OK;
+    return build_permuted(c, vol_dev, (cudaStream_t)stream);
+}
+
+static void fill_layouts(const fp_ctx *c, const float *vol, bool use_perm, AxisLayout lay[3])
+{
+    const long long nx = c->G.n[0], ny = c->G.n[1], nz = c->G.n[2];
+    // m = x: slices [x], slow y, fast z
+    lay[0] = AxisLayout{vol, ny * nz, nz, 1, (int)nx, (int)ny, (int)nz, 0};
+    // m = y: slices [y], slow x, fast z
+    lay[1] = AxisLayout{vol, nz, ny * nz, 1, (int)ny, (int)nx, (int)nz, 0};
+    // m = z: slow x, fast y; permuted copy [nz][nx][ny] when built
+    if (use_perm)
+        lay[2] = AxisLayout{c->vol_perm, nx * ny, ny, 1, (int)nz, (int)nx, (int)ny, 0};
+    else
+        lay[2] = AxisLayout{vol, 1, ny * nz, nz, (int)nz, (int)nx, (int)ny, 0};
+}
+
+static fp_status check_project_args(fp_ctx *c, const void *vol, int n_proj, const double *geom, int nu, int nv,
+                                    const void *out)
+{
+    if (!c) return FP_ERR_INVALID_ARG;
+    if (n_proj < 0) return fail(c, FP_ERR_INVALID_ARG, "n_proj < 0");
+    if (nu < 1 || nv < 1) return fail(c, FP_ERR_INVALID_ARG, "nu, nv must be >= 1");
+    if (n_proj > 0 && (!vol || !geom || !out)) return fail(c, FP_ERR_INVALID_ARG, "null pointer");
+    if (n_proj > 65535) return fail(c, FP_ERR_UNSUPPORTED, "n_proj > 65535 per call: split the call");
+    return FP_OK;
+}
+
+extern "C" fp_status fp_project(fp_ctx *c, const float *vol_dev, int n_proj, const double *geom, int nu, int nv,
+                                float *out_dev, fp_stream stream)
+{
+    fp_status s = check_project_args(c, vol_dev, n_proj, geom, nu, nv, out_dev);
+    if (s != FP_OK) return s;
+    cudaStream_t st = (cudaStream_t)stream;
+    c->last_launches = 0;
+    c->last_stream = st;
+    c->counted = false;
+    if (n_proj == 0) return FP_OK;
+
+    // layout stage: only when some projection has z-driven rays
+    bool want_perm = false;
+    if (c->opt_permuted)
+        for (int p = 0; p < n_proj && !want_perm; ++p) want_perm = has_z_driven(geom + 12 * (size_t)p, nu, nv);
+    if (want_perm && (!c->perm_valid || c->perm_src != vol_dev || c->opt_volatile)) {
+        s = build_permuted(c, vol_dev, st);
+        if (s != FP_OK) return s;
+    }
+    const bool use_perm = want_perm && c->perm_valid;
+
+    s = upload_geometry(c, n_proj, geom, nu, nv, use_perm, st);
+    if (s != FP_OK) return s;
+
+    ProjectParams P;
+    P.G = c->G;
+    fill_layouts(c, vol_dev, use_perm, P.lay);
+    P.proj = c->proj_dev;
+    P.out = out_dev;
+    P.sample_count = nullptr;
+    P.nu = nu;
+    P.nv = nv;
+    P.n_proj = n_proj;
+    P.interp = c->opt_interp;
+    if (c->opt_count) {
+        if (!c->count_dev) FP_CUDA(c, cudaMalloc(&c->count_dev, sizeof(unsigned long long)));
+        FP_CUDA(c, cudaMemsetAsync(c->count_dev, 0, sizeof(unsigned long long), st));
+        P.sample_count = c->count_dev;
+        c->counted = true;
+    }
+
+    const unsigned gl = (unsigned)((std::max(nu, nv) + kTileLane - 1) / kTileLane);
+    const unsigned gr = (unsigned)((std::max(nu, nv) + kTileRow - 1) / kTileRow);
+    dim3 grid(gl, gr, (unsigned)n_proj);
+    if (c->opt_interp == FP_INTERP_SPLINE)
+        fp_direct_kernel<1><<<grid, kDirectThreads, 0, st>>>(P);
+    else
+        fp_direct_kernel<0><<<grid, kDirectThreads, 0, st>>>(P);
+    FP_CUDA(c, cudaGetLastError());
+    c->last_launches += 1;
+    return FP_OK;
+}
+
+extern "C" fp_status fp_ray_ranges(fp_ctx *c, int n_proj, const double *geom, int nu, int nv, int32_t *mfl_dev,
+                                   fp_stream stream)
+{
+    fp_status s = check_project_args(c, mfl_dev, n_proj, geom, nu, nv, mfl_dev);
+    if (s != FP_OK) return s;
+    if (n_proj == 0) return FP_OK;
+    cudaStream_t st = (cudaStream_t)stream;
+    s = upload_geometry(c, n_proj, geom, nu, nv, false, st);
+    if (s != FP_OK) return s;
+    dim3 grid((unsigned)((nu + 31) / 32), (unsigned)((nv + 7) / 8), (unsigned)n_proj);
+    fp_ranges_kernel<<<grid, 256, 0, st>>>(c->G, c->proj_dev, nu, nv, mfl_dev);
+    FP_CUDA(c, cudaGetLastError());
+    return FP_OK;
+}
+
+extern "C" fp_status fp_last_sample_count(fp_ctx *c, unsigned long long *n)
+{
+    if (!c || !n) return FP_ERR_INVALID_ARG;
+    *n = 0;
+    if (!c->counted || !c->count_dev) return fail(c, FP_ERR_INVALID_ARG, "no counted fp_project call to report");
+    FP_CUDA(c, cudaStreamSynchronize(c->last_stream));
+    FP_CUDA(c, cudaMemcpy(n, c->count_dev, sizeof(unsigned long long), cudaMemcpyDeviceToHost));
+    return FP_OK;
+}
+
+extern "C" fp_status fp_last_launch_count(fp_ctx *c, int *n)
+{
+    if (!c || !n) return FP_ERR_INVALID_ARG;
+    *n = c->last_launches;
+    return FP_OK;
+}
+
+// End-to-end entry point: host volume in, host projections out.  The volume goes up once; the
+// projections are computed in batches on two streams so that the device-to-host copy of one
+// batch overlaps the kernels of the next.
+extern "C" fp_status fp_project_host(fp_ctx *c, const float *vol_host, int n_proj, const double *geom, int nu,
+                                     int nv, float *out_host)
+{
+    fp_status s = check_project_args(c, vol_host, n_proj, geom, nu, nv, out_host);
+    if (s != FP_OK) return s;
+    if (n_proj == 0) return FP_OK;
+    const size_t nvox = n_voxels(c);
+    const size_t per_proj = (size_t)nu * nv;
+    int batch = (int)std::max<size_t>(1, std::min<size_t>((size_t)n_proj, ((size_t)256 << 20) / (per_proj * sizeof(float))));
+    for (int k = 0; k < 2; ++k) {
+        if (!c->hstream[k]) FP_CUDA(c, cudaStreamCreateWithFlags(&c->hstream[k], cudaStreamNonBlocking));
+        if (!c->hevent[k]) FP_CUDA(c, cudaEventCreateWithFlags(&c->hevent[k], cudaEventDisableTiming));
+    }
+    if (!c->hvol_dev) FP_CUDA(c, cudaMalloc(&c->hvol_dev, nvox * sizeof(float)));
+    if (c->hout_cap < (size_t)batch * per_proj) {
+        for (int k = 0; k < 2; ++k) {
+            cudaFree(c->hout_dev[k]);
+            c->hout_dev[k] = nullptr;
+            FP_CUDA(c, cudaMalloc(&c->hout_dev[k], (size_t)batch * per_proj * sizeof(float)));
+        }
+        c->hout_cap = (size_t)batch * per_proj;
+    }
+    FP_CUDA(c, cudaMemcpyAsync(c->hvol_dev, vol_host, nvox * sizeof(float), cudaMemcpyHostToDevice, c->hstream[0]));
+    FP_CUDA(c, cudaEventRecord(c->hevent[0], c->hstream[0]));
+    FP_CUDA(c, cudaStreamWaitEvent(c->hstream[1], c->hevent[0], 0));
+    // the layout copy (if any) is made once, then kept for all batches
+    const int was_volatile = c->opt_volatile;
+    unsigned long long total = 0;
+    int launches = 0;
+    bool first = true;
+    for (int p0 = 0, b = 0; p0 < n_proj; p0 += batch, ++b) {
+        const int k = b & 1;
+        const int np = std::min(batch, n_proj - p0);
+        if (!first) c->opt_volatile = 0;
+        // each batch's kernel has finished (host sync below) before the next batch is planned, so the
+        // shared geometry buffer is free; only the device-to-host copies overlap the next kernels
+        s = fp_project(c, c->hvol_dev, np, geom + 12 * (size_t)p0, nu, nv, c->hout_dev[k], c->hstream[k]);
+        c->opt_volatile = was_volatile;
+        if (s != FP_OK) return s;
+        launches += c->last_launches;
+        first = false;
+        if (c->opt_count) {
+            unsigned long long n = 0;
+            s = fp_last_sample_count(c, &n);      // synchronises this batch's stream
+            if (s != FP_OK) return s;
+            total += n;
+        } else {
+            FP_CUDA(c, cudaStreamSynchronize(c->hstream[k]));
+        }
+        FP_CUDA(c, cudaMemcpyAsync(out_host + (size_t)p0 * per_proj, c->hout_dev[k], (size_t)np * per_proj * sizeof(float),
+                                   cudaMemcpyDeviceToHost, c->hstream[k]));
+    }
+    FP_CUDA(c, cudaStreamSynchronize(c->hstream[0]));
+    FP_CUDA(c, cudaStreamSynchronize(c->hstream[1]));
+    c->last_launches = launches;
+    if (c->opt_count) {
+        // leave the total where fp_last_sample_count finds it
+        FP_CUDA(c, cudaMemcpy(c->count_dev, &total, sizeof total, cudaMemcpyHostToDevice));
+        c->last_stream = c->hstream[0];
+        c->counted = true;
+    }
+    return FP_OK;
+}

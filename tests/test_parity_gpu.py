@@ -1,0 +1,286 @@
+"""GPU parity: libfp.so (through the C ABI binding) against the fp64 oracle, element by element,
+on the same seeded inputs.  Tolerance (BASELINE.json north_star): per ray
+|gpu - oracle| <= 2e-5 |oracle| + 1e-6 * path length * max|voxel|; (m, i_first, i_last) exact."""
+import math
+
+import numpy as np
+import pytest
+
+from parity_util import assert_parity
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def torch():
+    import torch as t
+    assert t.cuda.is_available()
+    return t
+
+
+@pytest.fixture(scope="module")
+def fp():
+    from paper_1609_00958_b200 import fp as m
+    m.load()
+    return m
+
+
+@pytest.fixture(scope="module")
+def synth():
+    from paper_1609_00958_b200 import synth as s
+    return s
+
+
+def all_ids(n_proj, nv, nu, projs=None):
+    projs = range(n_proj) if projs is None else projs
+    p, v, u = np.meshgrid(np.array(list(projs)), np.arange(nv), np.arange(nu), indexing="ij")
+    return np.stack([p.ravel(), v.ravel(), u.ravel()], axis=1).astype(np.int32)
+
+
+def run_gpu(torch, fp, vol_np, delta, origin, geom, nu, nv, options=()):
+    vol = torch.from_numpy(np.ascontiguousarray(vol_np, dtype=np.float32)).cuda()
+    with fp.Projector(*vol_np.shape, delta, origin) as P:
+        for k, v in options:
+            P.set_option(k, v)
+        out = P.project(vol, geom, nu, nv)
+        mfl = P.ray_ranges(geom, nu, nv)
+        torch.cuda.synchronize()
+        n = P.last_sample_count()
+        return out.cpu().numpy(), mfl.cpu().numpy(), n
+
+
+def compare_full(torch, fp, oracle, vol_np, delta, origin, geom, nu, nv, options=(), kernel=0, what=""):
+    geom = np.asarray(geom, dtype=np.float64).reshape(-1, 12)
+    out, mfl, n = run_gpu(torch, fp, vol_np, delta, origin, geom, nu, nv, options)
+    ids = all_ids(geom.shape[0], nv, nu)
+    ov, om, pl, mg = oracle.project_rays(vol_np, delta, origin, geom, ids, kernel=kernel, threads=oracle.host_cores())
+    worst = assert_parity(out.ravel(), mfl.reshape(-1, 3), ov, om, pl, mg, float(np.abs(vol_np).max()), what)
+    assert n == int(np.maximum(om[:, 2] - om[:, 1] + 1, 0).sum()), "sample count"
+    return worst, out, om
+
+
+# ----------------------------------------------------------------------------- BASELINE configs
+
+def test_c1_tiny_cone_beam_full(torch, fp, synth, oracle):
+    cfg = synth.CONFIGS["C1"]
+    vol = synth.make_volume(cfg).numpy()
+    geom = synth.make_geometry(cfg)
+    worst, out, om = compare_full(torch, fp, oracle, vol, cfg.voxel_size, cfg.origin, geom, cfg.nu, cfg.nv, what="C1")
+    assert out.shape == (16, 48, 48) and worst < 1.0
+    assert set(np.unique(om[:, 0])) == {0, 1}
+
+
+def test_c2_128_cube_full_orbit(torch, fp, synth, oracle):
+    cfg = synth.CONFIGS["C2"]
+    vol = synth.make_volume(cfg).numpy()
+    geom = synth.make_geometry(cfg)
+    out, mfl, n = run_gpu(torch, fp, vol, cfg.voxel_size, cfg.origin, geom, cfg.nu, cfg.nv)
+    # every ray of 12 projections (including the driving-axis switches at 45 deg + k 90 deg) ...
+    projs = [0, 22, 23, 44, 45, 67, 68, 90, 113, 135, 158, 179]
+    ids = all_ids(cfg.n_proj, cfg.nv, cfg.nu, projs)
+    # ... plus 2^18 random rays over the whole orbit
+    ids = np.concatenate([ids, synth.sample_rays(cfg, 1 << 18)])
+    ov, om, pl, mg = oracle.project_rays(vol, cfg.voxel_size, cfg.origin, geom, ids, threads=oracle.host_cores())
+    g = out[ids[:, 0], ids[:, 1], ids[:, 2]]
+    gm = mfl[ids[:, 0], ids[:, 1], ids[:, 2]]
+    assert assert_parity(g, gm, ov, om, pl, mg, float(np.abs(vol).max()), "C2") < 1.0
+    assert n == int(np.maximum(mfl[..., 2] - mfl[..., 1] + 1, 0).sum())
+
+
+def _big_config_subset(torch, fp, synth, oracle, name, projs, n_random, batch=None):
+    """Full-size volume on the device, the launch configuration bench.py times (whole batches
+    through fp_project), compared on sampled rays the oracle computes one by one."""
+    cfg = synth.CONFIGS[name]
+    vol_t = synth.make_volume(cfg, device="cuda")
+    vol = vol_t.cpu().numpy()
+    geom = synth.make_geometry(cfg)
+    sub = geom[projs]
+    with fp.Projector(*cfg.n, cfg.voxel_size, cfg.origin) as P:
+        out = P.project(vol_t, sub, cfg.nu, cfg.nv)
+        mfl = P.ray_ranges(sub, cfg.nu, cfg.nv)
+        torch.cuda.synchronize()
+        n = P.last_sample_count()
+        out, mfl = out.cpu().numpy(), mfl.cpu().numpy()
+    rng = np.random.default_rng(cfg.seed + 77)
+    ids = np.stack([rng.integers(0, len(projs), n_random), rng.integers(0, cfg.nv, n_random),
+                    rng.integers(0, cfg.nu, n_random)], axis=1).astype(np.int32)
+    # one full detector row and column per projection as well (tile edges, ragged tails)
+    extra = []
+    for p in range(len(projs)):
+        extra += [(p, cfg.nv // 3, u) for u in range(cfg.nu)] + [(p, v, cfg.nu - 1) for v in range(cfg.nv)]
+    ids = np.concatenate([ids, np.array(extra, dtype=np.int32)])
+    ov, om, pl, mg = oracle.project_rays(vol, cfg.voxel_size, cfg.origin, sub, ids, threads=oracle.host_cores())
+    g = out[ids[:, 0], ids[:, 1], ids[:, 2]]
+    gm = mfl[ids[:, 0], ids[:, 1], ids[:, 2]]
+    worst = assert_parity(g, gm, ov, om, pl, mg, float(np.abs(vol).max()), name)
+    assert n == int(np.maximum(mfl[..., 2] - mfl[..., 1] + 1, 0).sum())
+    return worst, om
+
+
+def test_c3_paper_scale_sampled(torch, fp, synth, oracle):
+    worst, om = _big_config_subset(torch, fp, synth, oracle, "C3", [0, 44, 45, 46, 90, 135, 201, 359], 60000)
+    assert worst < 1.0 and set(np.unique(om[:, 0])) == {0, 1}
+
+
+def test_c4_wide_cone_general_poses_sampled(torch, fp, synth, oracle):
+    worst, om = _big_config_subset(torch, fp, synth, oracle, "C4", [0, 1, 2, 3, 100, 255], 60000)
+    assert worst < 1.0
+    assert set(np.unique(om[:, 0])) == {0, 1, 2}          # all three driving axes
+    assert (om[:, 2] < om[:, 1]).mean() > 0.05            # and a fair share of misses
+
+
+def test_c5_large_volume_sampled(torch, fp, synth, oracle):
+    worst, om = _big_config_subset(torch, fp, synth, oracle, "C5", [0, 89, 90, 91, 400, 719], 40000)
+    assert worst < 1.0
+
+
+# ----------------------------------------------------------------------------- edge cases
+
+def small_problem(rng, shape=(19, 13, 23), delta=0.7):
+    vol = rng.uniform(-1.0, 2.0, size=shape).astype(np.float32)
+    origin = tuple(-(n - 1) / 2.0 * delta + 0.3 * k for k, n in enumerate(shape))
+    return vol, delta, origin
+
+
+def pose(src, look_at, nu, nv, pitch, sdd, roll=0.0):
+    src = np.asarray(src, float)
+    n = np.asarray(look_at, float) - src
+    n /= np.linalg.norm(n)
+    ax = np.zeros(3)
+    ax[int(np.argmin(np.abs(n)))] = 1.0
+    e1 = np.cross(n, ax)
+    e1 /= np.linalg.norm(e1)
+    e2 = np.cross(n, e1)
+    U = pitch * (math.cos(roll) * e1 + math.sin(roll) * e2)
+    V = pitch * (-math.sin(roll) * e1 + math.cos(roll) * e2)
+    C = src + sdd * n
+    O = C - (nu - 1) / 2.0 * U - (nv - 1) / 2.0 * V
+    return np.concatenate([src, O, U, V])
+
+
+@pytest.mark.parametrize("nu,nv", [(1, 1), (37, 53), (33, 9), (8, 65)])
+def test_ragged_detectors_and_anisotropic_grid_all_axes(torch, fp, oracle, nu, nv):
+    rng = np.random.default_rng(100 + nu)
+    vol, delta, origin = small_problem(rng)
+    geom = np.stack([pose(s, (0.2, -0.1, 0.3), nu, nv, 0.5, 60.0, roll)
+                     for s, roll in [((-30, 2, 1), 0.0), ((1, 28, -3), 0.4), ((2, -1, 31), 1.1),
+                                     ((-14, -15, 16), 2.0), ((20, 3, -19), 0.7)]])
+    for perm in (1, 0):
+        worst, _, om = compare_full(torch, fp, oracle, vol, delta, origin, geom, nu, nv,
+                                    options=[(fp.OPT_PERMUTED_COPY, perm)], what="ragged %dx%d perm=%d" % (nu, nv, perm))
+        assert worst < 1.0
+    if nu * nv > 100:
+        assert set(np.unique(om[:, 0])) == {0, 1, 2}
+
+
+def test_spline_kernel(torch, fp, oracle):
+    rng = np.random.default_rng(5)
+    vol, delta, origin = small_problem(rng)
+    geom = np.stack([pose((-30, 4, 2), (0, 0, 0), 40, 24, 0.45, 60.0, 0.3), pose((3, 4, 29), (0, 0, 0), 40, 24, 0.45, 55.0, 0.0)])
+    worst, _, _ = compare_full(torch, fp, oracle, vol, delta, origin, geom, 40, 24,
+                               options=[(fp.OPT_INTERP, fp.INTERP_SPLINE)], kernel=1, what="spline")
+    assert worst < 1.0
+
+
+def test_all_rays_miss_and_n_proj_zero(torch, fp, oracle):
+    rng = np.random.default_rng(6)
+    vol, delta, origin = small_problem(rng)
+    geom = pose((-30, 200, 2), (0, 400, 0), 16, 16, 0.5, 60.0)[None]       # looks away from the volume
+    worst, out, om = compare_full(torch, fp, oracle, vol, delta, origin, geom, 16, 16, what="miss")
+    assert np.all(out == 0.0) and np.all(om[:, 2] < om[:, 1])
+    volt = torch.from_numpy(vol).cuda()
+    with fp.Projector(*vol.shape, delta, origin) as P:
+        out = P.project(volt, np.zeros((0, 12)), 16, 16)
+        assert out.shape == (0, 16, 16)
+
+
+def test_axis_parallel_rays_ties_and_degenerate_ray(torch, fp, oracle):
+    """Rays exactly parallel to an axis (r~_t = 0), exact |r| ties (lowest axis wins, reading #8),
+    integer sample positions (second tap weight 0) and a pixel that coincides with the
+    source (r = 0 -> output 0)."""
+    vol = np.arange(6 * 5 * 4, dtype=np.float32).reshape(6, 5, 4) / 8.0
+    delta, origin = 1.0, (0.0, 0.0, 0.0)
+    rows = []
+    # parallel-ish fan: source far on -x, detector plane x = 10, pixel centres on integer (y, z)
+    rows.append(np.array([-1e6, 2.0, 1.0, 10.0, 0.0, 0.0, 0.0, 1.0, 0.0, 0.0, 0.0, 1.0]))
+    # source on the x axis: the central pixel's ray is exactly axis-parallel
+    rows.append(np.array([-20.0, 2.0, 1.0, 10.0, 0.0, -1.0, 0.0, 1.0, 0.0, 0.0, 0.0, 1.0]))
+    # exact ties |r_x| = |r_y| on the diagonal pixels
+    rows.append(np.array([-8.0, -8.0, 1.5, -6.0, -6.0, 1.5, 0.0, 1.0, 0.0, 1.0, 0.0, 0.0]))
+    # detector plane through the source: pixel (2,1) is the source itself
+    rows.append(np.array([3.0, 2.0, 9.0, 1.0, 1.0, 9.0, 1.0, 0.0, 0.0, 0.0, 1.0, 0.0]))
+    geom = np.stack(rows)
+    worst, out, om = compare_full(torch, fp, oracle, vol, delta, origin, geom, 6, 5, what="axis-parallel")
+    assert worst < 1.0
+    assert out[3, 1, 2] == 0.0
+
+
+def test_single_slice_and_single_voxel_volumes(torch, fp, oracle):
+    rng = np.random.default_rng(8)
+    for shape in [(1, 9, 7), (9, 1, 7), (9, 7, 1), (1, 1, 1)]:
+        vol = rng.uniform(0.5, 1.5, size=shape).astype(np.float32)
+        origin = tuple(-(n - 1) / 2.0 for n in shape)
+        geom = np.stack([pose((-25, 1, 2), (0, 0, 0), 24, 20, 0.6, 50.0), pose((2, 1, 25), (0, 0, 0), 24, 20, 0.6, 50.0),
+                         pose((1, -25, 2), (0, 0, 0), 24, 20, 0.6, 50.0)])
+        worst, _, _ = compare_full(torch, fp, oracle, vol, 1.0, origin, geom, 24, 20, what=str(shape))
+        assert worst < 1.0
+
+
+def test_constant_volume_chord_property_at_full_size(torch, fp):
+    """A property that holds at any size (no oracle needed): for a constant volume every ray that
+    enters and leaves through the driving-axis faces returns c * delta * ||r~|| * N_m."""
+    n = 512
+    vol = torch.full((n, n, n), 0.5, device="cuda", dtype=torch.float32)
+    from paper_1609_00958_b200 import synth
+    cfg = synth.CONFIGS["C3"]
+    geom = synth.make_geometry(cfg)[[10]]
+    with fp.Projector(n, n, n, 1.0, cfg.origin) as P:
+        out = P.project(vol, geom, cfg.nu, cfg.nv).cpu().numpy()[0]
+        mfl = P.ray_ranges(geom, cfg.nu, cfg.nv).cpu().numpy()[0]
+    full = (mfl[..., 1] == 0) & (mfl[..., 2] == n - 1)
+    assert full.mean() > 0.3
+    # ||r~|| recomputed here from the geometry
+    g = geom[0]
+    iv, iu = np.meshgrid(np.arange(cfg.nv), np.arange(cfg.nu), indexing="ij")
+    D = g[3:6][None, None] + iu[..., None] * g[6:9] + iv[..., None] * g[9:12]
+    r = D - g[0:3]
+    L = np.linalg.norm(r, axis=-1) / np.abs(r).max(axis=-1)
+    # interior rays only (all four taps inside on every slice): compare where the value is the chord
+    expect = 0.5 * L * n
+    inner = full & (np.abs(out - expect) <= 2e-5 * expect + 1e-6 * L * n * 0.5)
+    # rays whose transverse range touches the zero padding have smaller values; all others must match
+    assert np.all(out[full] <= expect[full] * (1 + 3e-5))
+    assert inner.sum() > 0.25 * full.size
+
+
+def test_project_host_matches_device_path(torch, fp, synth):
+    cfg = synth.CONFIGS["C1"]
+    vol = synth.make_volume(cfg)
+    geom = synth.make_geometry(cfg)
+    with fp.Projector(*cfg.n, cfg.voxel_size, cfg.origin) as P:
+        a = P.project(vol.cuda(), geom, cfg.nu, cfg.nv).cpu()
+        n1 = P.last_sample_count()
+        b = P.project_host(vol.pin_memory(), geom, cfg.nu, cfg.nv)
+        n2 = P.last_sample_count()
+    assert torch.equal(a, b) and n1 == n2
+
+
+def test_reuse_context_changed_volume_and_streams(torch, fp, synth, oracle):
+    """The volume changes between calls (iterative reconstruction): with the default
+    FP_OPT_VOLATILE = 1 the z-driven layout copy is rebuilt; work runs on a caller's stream."""
+    rng = np.random.default_rng(9)
+    vol, delta, origin = small_problem(rng)
+    geom = np.stack([pose((2, -1, 31), (0, 0, 0), 32, 32, 0.5, 60.0, 0.2)])
+    ids = all_ids(1, 32, 32)
+    s = torch.cuda.Stream()
+    with fp.Projector(*vol.shape, delta, origin) as P:
+        for scale in (1.0, -2.0):
+            v = (vol * scale).astype(np.float32)
+            vt = torch.from_numpy(v).cuda()
+            torch.cuda.synchronize()
+            with torch.cuda.stream(s):
+                out = P.project(vt, geom, 32, 32, stream=s)
+            s.synchronize()
+            ov, om, pl, mg = oracle.project_rays(v, delta, origin, geom, ids)
+            gm = P.ray_ranges(geom, 32, 32).cpu().numpy()
+            assert assert_parity(out.cpu().numpy().ravel(), gm.reshape(-1, 3), ov, om, pl, mg, float(np.abs(v).max())) < 1.0
