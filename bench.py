@@ -215,15 +215,17 @@ def main():
         if dist is not None:
             dist.barrier()
 
-    for _ in range(args.warmup):
-        step()
-    torch.cuda.synchronize()
-    # sample count of one step (outside the timed region: fp_last_sample_count synchronises)
+    # sample count of one step (outside the timed region: fp_last_sample_count synchronises, and the
+    # count costs one exact fp64 ray set-up per ray that the sampling itself does not need)
     samples = 0
     for p0 in range(0, cfg.n_proj, batch):
         p1 = min(cfg.n_proj, p0 + batch)
         P.project(vol, geom[p0:p1], cfg.nu, cfg.nv, out=out[p0:p1], stream=stream)
         samples += P.last_sample_count()
+    P.set_option(fp.OPT_COUNT_SAMPLES, 0)
+    for _ in range(args.warmup):
+        step()
+    torch.cuda.synchronize()
 
     ev = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps + 1)]
     barrier()
@@ -287,7 +289,7 @@ def main():
     achieved = algo_bytes_per_step / (kernel_ms * 1e-3) / 1e9
     roofline = {"bound": "hbm", "achieved": achieved, "peak": peaks["hbm_gbs"], "unit": "GB/s",
                 "frac": achieved / peaks["hbm_gbs"], "traffic": None, "peak_kind": peak_kind,
-                "kernel": "fp_direct_kernel", "algorithmic_bytes_per_launch": algo_bytes_per_step // max(1, (cfg.n_proj + batch - 1) // batch)}
+                "kernel": "fp_aligned_kernel" if (cfg.orbit == "circular" and args.kernel != 1) else "fp_direct_kernel", "algorithmic_bytes_per_launch": algo_bytes_per_step // max(1, (cfg.n_proj + batch - 1) // batch)}
 
     cpu_baseline = None
     parity = None

@@ -62,7 +62,12 @@ typedef enum {
 
 /* fp_set_option keys.  Options are explicit; no environment variable changes behaviour. */
 enum {
-    /* Sampling-kernel variant: FP_KERNEL_AUTO picks per projection. */
+    /* Sampling-kernel variant.  FP_KERNEL_AUTO picks per projection: FP_KERNEL_ALIGNED (line
+     * staging in shared memory) for poses whose v vector is parallel to the volume's z axis and
+     * whose u vector is perpendicular to it and that have no z-driven ray (every circular orbit
+     * about z), FP_KERNEL_DIRECT (one thread per ray, four global taps per
+     * sample) for every other pose.  FP_KERNEL_DIRECT forces the direct kernel for all poses;
+     * FP_KERNEL_ALIGNED behaves like AUTO (poses it cannot take still use the direct kernel). */
     FP_OPT_KERNEL = 1,
     /* 1 (default): the volume contents may have changed since the last call, internal copies
      * are rebuilt by every fp_project that needs them.  0: internal copies made by fp_prepare
@@ -80,7 +85,7 @@ enum {
     FP_OPT_COUNT_SAMPLES = 5
 };
 
-enum { FP_KERNEL_AUTO = 0, FP_KERNEL_DIRECT = 1, FP_KERNEL_STAGED = 2 };
+enum { FP_KERNEL_AUTO = 0, FP_KERNEL_DIRECT = 1, FP_KERNEL_ALIGNED = 2 };
 enum { FP_INTERP_LINEAR = 0, FP_INTERP_SPLINE = 1 };
 
 /*

@@ -13,6 +13,7 @@
 
 #include "../../include/fp.h"
 #include "fp_kernels.cuh"
+#include "fp_aligned.cuh"
 
 using namespace fpk;
 
@@ -31,7 +32,10 @@ struct fp_ctx {
     // per-call workspaces
     ProjDesc *proj_dev = nullptr;
     int proj_cap = 0;
-    unsigned long long *count_dev = nullptr;
+    unsigned long long *count_dev = nullptr;   // [0] sample count, [1] (low word) staging-window error flag
+    int *ids_dev = nullptr;                    // [2 * ids_cap]: aligned ids, then direct ids
+    int ids_cap = 0;
+    bool aligned_attr_set = false;
     cudaStream_t last_stream = nullptr;
     bool counted = false;
     int last_launches = 0;
@@ -110,6 +114,7 @@ extern "C" fp_status fp_destroy(fp_ctx *c)
     cudaFree(c->vol_perm);
     cudaFree(c->proj_dev);
     cudaFree(c->count_dev);
+    cudaFree(c->ids_dev);
     cudaFree(c->hvol_dev);
     for (int k = 0; k < 2; ++k) {
         cudaFree(c->hout_dev[k]);
@@ -126,8 +131,7 @@ extern "C" fp_status fp_set_option(fp_ctx *c, int key, int value)
     if (!c) return FP_ERR_INVALID_ARG;
     switch (key) {
     case FP_OPT_KERNEL:
-        if (value < FP_KERNEL_AUTO || value > FP_KERNEL_STAGED) return fail(c, FP_ERR_INVALID_ARG, "bad kernel variant");
-        if (value == FP_KERNEL_STAGED) return fail(c, FP_ERR_UNSUPPORTED, "staged kernel not built yet");
+        if (value < FP_KERNEL_AUTO || value > FP_KERNEL_ALIGNED) return fail(c, FP_ERR_INVALID_ARG, "bad kernel variant");
         c->opt_kernel = value;
         return FP_OK;
     case FP_OPT_VOLATILE: c->opt_volatile = value != 0; return FP_OK;
@@ -217,6 +221,81 @@ static int plan_lane_v(const double *g, int nu, int nv, bool permuted)
     if (m == 2 && !permuted) return std::fabs(g[9 + 1]) > std::fabs(g[6 + 1]);
     return std::fabs(g[9 + fast]) > std::fabs(g[6 + fast]);
 }
+
+// Can fp_aligned_kernel take this pose, and how wide a staging window (voxels along z) does it
+// need?  Conditions: u perpendicular to z, v parallel to z (exact zeros, so that r_x, r_y depend
+// on the column only and r_z on the row only), no z-driven ray, nz a multiple of 4 and a
+// 16-byte aligned volume (float4 loads along z).  The window bound is conservative: the largest
+// ray parameter |t| = |(i - s_m) / r_m| over all slices a batch can touch, times the r_z spread
+// of the rows of one block, plus the drift inside a batch, alignment and tap margins.
+static int plan_aligned(const fp_ctx *c, const float *vol, const double *g, int nu, int nv)
+{
+    for (int k = 0; k < 12; ++k)
+        if (!std::isfinite(g[k])) return 0;
+    if (g[8] != 0.0 || g[9] != 0.0 || g[10] != 0.0 || g[11] == 0.0) return 0;
+    if ((c->G.n[2] & 3) != 0 || ((uintptr_t)vol & 15) != 0) return 0;
+    const double dl = c->G.delta;
+    double s[3];
+    for (int a = 0; a < 3; ++a) s[a] = (g[a] - c->G.origin[a]) / dl;
+    auto rho = [&](int iv) { return ((g[5] + iv * g[11]) - c->G.origin[2]) / dl - s[2]; };
+    const double rz_max = std::max(std::fabs(rho(0)), std::fabs(rho(nv - 1)));
+    double rm_min = INFINITY, t_max = 0.0;
+    for (int iu = 0; iu < nu; ++iu) {
+        double r[2];
+        for (int a = 0; a < 2; ++a) r[a] = ((g[3 + a] + iu * g[6 + a]) - c->G.origin[a]) / dl - s[a];
+        const int m = std::fabs(r[1]) > std::fabs(r[0]) ? 1 : 0;
+        const double rm = r[m];
+        rm_min = std::min(rm_min, std::fabs(rm));
+        if (rm == 0.0) return 0;
+        const double t_a = (0.0 - s[m]) / rm, t_b = ((double)(c->G.n[m] - 1 + kAlSB) - s[m]) / rm;
+        t_max = std::max(t_max, std::max(std::fabs(t_a), std::fabs(t_b)));
+    }
+    if (!(rz_max <= rm_min * (1.0 - 1e-9))) return 0;            // a z-driven (or tied) ray somewhere
+    const int rows = std::min(nv, kAlTV);
+    const double span = t_max * (rows - 1) * std::fabs(g[11] / dl) + (kAlSB - 1) * (rz_max / rm_min);
+    if (!(span < 1.0e6)) return 0;
+    return (int)std::ceil(span) + 10;
+}
+
+static fp_status ensure_ids(fp_ctx *c, int n_proj)
+{
+    if (n_proj <= c->ids_cap) return FP_OK;
+    if (c->ids_dev) {
+        FP_CUDA(c, cudaDeviceSynchronize());
+        cudaFree(c->ids_dev);
+        c->ids_dev = nullptr;
+        c->ids_cap = 0;
+    }
+    const int cap = n_proj + 64;
+    FP_CUDA(c, cudaMalloc(&c->ids_dev, sizeof(int) * 2 * (size_t)cap));
+    c->ids_cap = cap;
+    return FP_OK;
+}
+
+template <int INTERP, int W>
+static fp_status launch_aligned_w(fp_ctx *c, const AlignedParams &A, dim3 grid, cudaStream_t st)
+{
+    constexpr size_t smem = aligned_smem_bytes<W>();
+    static bool attr_set = false;      // per process and instantiation; harmless to repeat
+    if (!attr_set) {
+        FP_CUDA(c, cudaFuncSetAttribute(fp_aligned_kernel<INTERP, W>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        attr_set = true;
+    }
+    fp_aligned_kernel<INTERP, W><<<grid, kAlTV, smem, st>>>(A);
+    FP_CUDA(c, cudaGetLastError());
+    return FP_OK;
+}
+
+template <int INTERP>
+static fp_status launch_aligned(fp_ctx *c, const AlignedParams &A, int w, dim3 grid, cudaStream_t st)
+{
+    if (w <= 128) return launch_aligned_w<INTERP, 128>(c, A, grid, st);
+    if (w <= 256) return launch_aligned_w<INTERP, 256>(c, A, grid, st);
+    if (w <= 384) return launch_aligned_w<INTERP, 384>(c, A, grid, st);
+    return launch_aligned_w<INTERP, 512>(c, A, grid, st);
+}
+
+constexpr int kAlignedMaxW = 512;
 
 static fp_status ensure_proj(fp_ctx *c, int n_proj)
 {
@@ -308,10 +387,24 @@ extern "C" fp_status fp_project(fp_ctx *c, const float *vol_dev, int n_proj, con
     c->counted = false;
     if (n_proj == 0) return FP_OK;
 
-    // layout stage: only when some projection has z-driven rays
+    // plan: which kernel takes which projection
+    std::vector<int> ids_al, ids_di;
+    int w_al = 0;
+    for (int p = 0; p < n_proj; ++p) {
+        const int w = c->opt_kernel == FP_KERNEL_DIRECT ? 0 : plan_aligned(c, vol_dev, geom + 12 * (size_t)p, nu, nv);
+        if (w > 0 && w <= kAlignedMaxW) {
+            ids_al.push_back(p);
+            w_al = std::max(w_al, w);
+        } else {
+            ids_di.push_back(p);
+        }
+    }
+
+    // layout stage: only when some projection of the direct kernel has z-driven rays
     bool want_perm = false;
     if (c->opt_permuted)
-        for (int p = 0; p < n_proj && !want_perm; ++p) want_perm = has_z_driven(geom + 12 * (size_t)p, nu, nv);
+        for (size_t q = 0; q < ids_di.size() && !want_perm; ++q)
+            want_perm = has_z_driven(geom + 12 * (size_t)ids_di[q], nu, nv);
     if (want_perm && (!c->perm_valid || c->perm_src != vol_dev || c->opt_volatile)) {
         s = build_permuted(c, vol_dev, st);
         if (s != FP_OK) return s;
@@ -320,33 +413,59 @@ extern "C" fp_status fp_project(fp_ctx *c, const float *vol_dev, int n_proj, con
 
     s = upload_geometry(c, n_proj, geom, nu, nv, use_perm, st);
     if (s != FP_OK) return s;
+    s = ensure_ids(c, n_proj);
+    if (s != FP_OK) return s;
+    if (!ids_al.empty())
+        FP_CUDA(c, cudaMemcpyAsync(c->ids_dev, ids_al.data(), sizeof(int) * ids_al.size(), cudaMemcpyHostToDevice, st));
+    if (!ids_di.empty())
+        FP_CUDA(c, cudaMemcpyAsync(c->ids_dev + c->ids_cap, ids_di.data(), sizeof(int) * ids_di.size(),
+                                   cudaMemcpyHostToDevice, st));
 
-    ProjectParams P;
-    P.G = c->G;
-    fill_layouts(c, vol_dev, use_perm, P.lay);
-    P.proj = c->proj_dev;
-    P.out = out_dev;
-    P.sample_count = nullptr;
-    P.nu = nu;
-    P.nv = nv;
-    P.n_proj = n_proj;
-    P.interp = c->opt_interp;
-    if (c->opt_count) {
-        if (!c->count_dev) FP_CUDA(c, cudaMalloc(&c->count_dev, sizeof(unsigned long long)));
-        FP_CUDA(c, cudaMemsetAsync(c->count_dev, 0, sizeof(unsigned long long), st));
-        P.sample_count = c->count_dev;
-        c->counted = true;
+    if (!c->count_dev) FP_CUDA(c, cudaMalloc(&c->count_dev, 2 * sizeof(unsigned long long)));
+    FP_CUDA(c, cudaMemsetAsync(c->count_dev, 0, 2 * sizeof(unsigned long long), st));
+    c->counted = c->opt_count != 0;
+
+    if (!ids_al.empty()) {
+        AlignedParams A;
+        A.G = c->G;
+        A.vol = vol_dev;
+        A.proj = c->proj_dev;
+        A.ids = c->ids_dev;
+        A.out = out_dev;
+        A.sample_count = c->opt_count ? c->count_dev : nullptr;
+        A.err_flag = reinterpret_cast<unsigned int *>(c->count_dev + 1);
+        A.nu = nu;
+        A.nv = nv;
+        A.n_sel = (int)ids_al.size();
+        dim3 grid((unsigned)((nu + kAlTU - 1) / kAlTU), (unsigned)((nv + kAlTV - 1) / kAlTV), (unsigned)ids_al.size());
+        s = c->opt_interp == FP_INTERP_SPLINE ? launch_aligned<1>(c, A, w_al, grid, st)
+                                              : launch_aligned<0>(c, A, w_al, grid, st);
+        if (s != FP_OK) return s;
+        c->last_launches += 1;
     }
 
-    const unsigned gl = (unsigned)((std::max(nu, nv) + kTileLane - 1) / kTileLane);
-    const unsigned gr = (unsigned)((std::max(nu, nv) + kTileRow - 1) / kTileRow);
-    dim3 grid(gl, gr, (unsigned)n_proj);
-    if (c->opt_interp == FP_INTERP_SPLINE)
-        fp_direct_kernel<1><<<grid, kDirectThreads, 0, st>>>(P);
-    else
-        fp_direct_kernel<0><<<grid, kDirectThreads, 0, st>>>(P);
-    FP_CUDA(c, cudaGetLastError());
-    c->last_launches += 1;
+    if (!ids_di.empty()) {
+        ProjectParams P;
+        P.G = c->G;
+        fill_layouts(c, vol_dev, use_perm, P.lay);
+        P.proj = c->proj_dev;
+        P.ids = c->ids_dev + c->ids_cap;
+        P.out = out_dev;
+        P.sample_count = c->opt_count ? c->count_dev : nullptr;
+        P.nu = nu;
+        P.nv = nv;
+        P.n_proj = (int)ids_di.size();
+        P.interp = c->opt_interp;
+        const unsigned gl = (unsigned)((std::max(nu, nv) + kTileLane - 1) / kTileLane);
+        const unsigned gr = (unsigned)((std::max(nu, nv) + kTileRow - 1) / kTileRow);
+        dim3 grid(gl, gr, (unsigned)ids_di.size());
+        if (c->opt_interp == FP_INTERP_SPLINE)
+            fp_direct_kernel<1><<<grid, kDirectThreads, 0, st>>>(P);
+        else
+            fp_direct_kernel<0><<<grid, kDirectThreads, 0, st>>>(P);
+        FP_CUDA(c, cudaGetLastError());
+        c->last_launches += 1;
+    }
     return FP_OK;
 }
 
@@ -371,7 +490,10 @@ extern "C" fp_status fp_last_sample_count(fp_ctx *c, unsigned long long *n)
     *n = 0;
     if (!c->counted || !c->count_dev) return fail(c, FP_ERR_INVALID_ARG, "no counted fp_project call to report");
     FP_CUDA(c, cudaStreamSynchronize(c->last_stream));
-    FP_CUDA(c, cudaMemcpy(n, c->count_dev, sizeof(unsigned long long), cudaMemcpyDeviceToHost));
+    unsigned long long h[2] = {0, 0};
+    FP_CUDA(c, cudaMemcpy(h, c->count_dev, sizeof h, cudaMemcpyDeviceToHost));
+    if (h[1] != 0) return fail(c, FP_ERR_CUDA, "internal error: a staging window of fp_aligned_kernel did not fit (host plan too small)");
+    *n = h[0];
     return FP_OK;
 }
 

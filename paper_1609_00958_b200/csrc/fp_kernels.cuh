@@ -27,6 +27,7 @@ struct ProjectParams {
     GridDesc G;
     AxisLayout lay[3];                 // indexed by the driving axis m
     const ProjDesc *proj;              // [n_proj]
+    const int *ids;                    // projections this launch handles (blockIdx.z -> projection), or null
     float *out;                        // [n_proj][nv][nu]
     unsigned long long *sample_count;  // may be null
     int nu, nv, n_proj;
@@ -69,7 +70,7 @@ template <int INTERP>
 __global__ void __launch_bounds__(kDirectThreads)
 fp_direct_kernel(const __grid_constant__ ProjectParams P)
 {
-    const int proj = blockIdx.z;
+    const int proj = P.ids ? P.ids[blockIdx.z] : (int)blockIdx.z;
     const ProjDesc *pd = P.proj + proj;
     const int lane = threadIdx.x & 31, row = threadIdx.x >> 5;
     const bool lane_v = pd->lane_v != 0;
