@@ -239,20 +239,41 @@ static int plan_aligned(const fp_ctx *c, const float *vol, const double *g, int 
     for (int a = 0; a < 3; ++a) s[a] = (g[a] - c->G.origin[a]) / dl;
     auto rho = [&](int iv) { return ((g[5] + iv * g[11]) - c->G.origin[2]) / dl - s[2]; };
     const double rz_max = std::max(std::fabs(rho(0)), std::fabs(rho(nv - 1)));
-    double rm_min = INFINITY, t_max = 0.0;
+    // per column: the slices whose slow-axis position can lie inside (-1, N_s) (one slice of slack on
+    // either side), widened by one batch; the ray parameter t = (i - s_m) / r_m over them
+    double rm_min = INFINITY, t_lo = INFINITY, t_hi = -INFINITY;
     for (int iu = 0; iu < nu; ++iu) {
         double r[2];
         for (int a = 0; a < 2; ++a) r[a] = ((g[3 + a] + iu * g[6 + a]) - c->G.origin[a]) / dl - s[a];
         const int m = std::fabs(r[1]) > std::fabs(r[0]) ? 1 : 0;
-        const double rm = r[m];
+        const double rm = r[m], rs = r[1 - m];
         rm_min = std::min(rm_min, std::fabs(rm));
         if (rm == 0.0) return 0;
-        const double t_a = (0.0 - s[m]) / rm, t_b = ((double)(c->G.n[m] - 1 + kAlSB) - s[m]) / rm;
-        t_max = std::max(t_max, std::max(std::fabs(t_a), std::fabs(t_b)));
+        double i_a = 0.0, i_b = (double)(c->G.n[m] - 1);
+        const double rt = rs / rm, ss = s[1 - m], ns = (double)c->G.n[1 - m];
+        if (rt != 0.0) {
+            const double x1 = s[m] + (-1.0 - ss) / rt, x2 = s[m] + (ns - ss) / rt;
+            i_a = std::max(i_a, std::floor(std::min(x1, x2)) - 1.0);
+            i_b = std::min(i_b, std::ceil(std::max(x1, x2)) + 1.0);
+        } else if (!(ss > -1.0 && ss < ns)) {
+            continue;
+        }
+        if (i_a > i_b) continue;
+        i_b += kAlSB;
+        const double t_a = (i_a - s[m]) / rm, t_b = (i_b - s[m]) / rm;
+        t_lo = std::min(t_lo, std::min(t_a, t_b));
+        t_hi = std::max(t_hi, std::max(t_a, t_b));
     }
     if (!(rz_max <= rm_min * (1.0 - 1e-9))) return 0;            // a z-driven (or tied) ray somewhere
+    if (!(t_lo <= t_hi)) return 16;                              // every column misses: any window will do
+    const double t_max = std::max(std::fabs(t_lo), std::fabs(t_hi));
     const int rows = std::min(nv, kAlTV);
-    const double span = t_max * (rows - 1) * std::fabs(g[11] / dl) + (kAlSB - 1) * (rz_max / rm_min);
+    // rows of one block at one t, the drift inside a batch, and the difference in t between the columns
+    // of a block, which share one window: their first slices differ (entry through a side face) and
+    // their r_m differ by at most kAlTU detector steps
+    const double du = std::max(std::fabs(g[6]), std::fabs(g[7])) / dl;
+    const double dt_cols = t_max * (kAlTU * du / rm_min) + 4.0 / rm_min;
+    const double span = t_max * (rows - 1) * std::fabs(g[11] / dl) + (kAlSB - 1) * (rz_max / rm_min) + dt_cols * rz_max;
     if (!(span < 1.0e6)) return 0;
     return (int)std::ceil(span) + 10;
 }

@@ -44,28 +44,33 @@ struct AlColumn {          // per detector column, constant over the slice loop
     long long stride_m, stride_s;      // element strides of the slice index and of the slow axis
     int i_lo, i_hi;        // slices with -1 < p_slow < N_slow (exact, clip_axis)
     int n_s, m;
+    int i_start, dir;      // slice of batch 0, step +1 / -1: slices are visited in order of ascending ray
+                           // parameter t = (i - s_m) / r_m, all columns of a block starting at the same t
 };
 
-struct AlLine {            // per staged line (column, slice of the batch)
+struct __align__(16) AlLine {   // per staged line (column, slice of the batch)
     const float *pa, *pb;  // rows j and j+1 at z = 0
     float u1;              // weight of row j+1
-    int z0f;               // window origin (multiple of 4) | 1 (row j inside) | 2 (row j+1 inside)
+    int flags;             // 1 (row j inside the volume) | 2 (row j+1 inside)
     int pad_[2];
 };
 
-struct AlBatch {           // per (column, batch): z position of the window in ray-parameter form
-    double t0;             // (i0 - s_m) / r_m at the batch's first slice
+struct __align__(16) AlBatch {  // per batch: the common z window of all its lines
     double off;            // s_z - z0
+    int z0, nq;            // window origin (multiple of 4), float4 quads to stage
 };
 
-struct AlShared {
+struct __align__(16) AlShared {
     AlColumn col[kAlTU];
     AlLine line[2][kAlNL];
-    AlBatch batch[2][kAlTU];
+    double t0[2][kAlTU];   // per (buffer, column): (i0 - s_m) / r_m at the batch's first slice
+    AlBatch batch[2];
     double s_z, rho_first, rho_last;
     int n_batches;
     unsigned lines_bias;   // shared-window byte address of the staged lines minus (0x4B000000 << 2)
 };
+
+static_assert(sizeof(AlShared) % 16 == 0 && sizeof(AlLine) == 32 && sizeof(AlBatch) == 16, "shared layout");
 
 template <int W>
 constexpr size_t aligned_smem_bytes() { return sizeof(AlShared) + sizeof(float) * (size_t)kAlNL * W; }
@@ -86,49 +91,56 @@ __device__ __forceinline__ float al_lds(unsigned addr)
     return v;
 }
 
-// Staging parameters of line l = (column c, slice s of batch b), written by one thread.
+__device__ __forceinline__ int al_to_int(double x)      // saturating double -> int
+{
+    return (int)fmin(fmax(x, -1.0e9), 1.0e9);
+}
+
+// Staging parameters of batch b, computed by warp 0: lane l = (column c, slice s) writes its line;
+// the z window is common to the whole batch (min / max over the 32 lines by warp reductions).
 template <int INTERP, int W>
-__device__ __forceinline__ void al_line_params(AlShared &S, const AlignedParams &P, int buf, int b, int l)
+__device__ __forceinline__ void al_batch_params(AlShared &S, const AlignedParams &P, int buf, int b, int l)
 {
     const int c = l / kAlSB, s = l - c * kAlSB;
     const AlColumn &C = S.col[c];
-    const int i0 = C.i_lo + b * kAlSB;
-    const int i = i0 + s;
-    // window origin of this (column, batch): the extreme rows at the first and at the last slice
-    const double ta = __dmul_rn(__dsub_rn((double)i0, C.s_m), C.inv_rm);
-    const double tb = __dmul_rn(__dsub_rn((double)(i0 + kAlSB - 1), C.s_m), C.inv_rm);
-    const double z1 = ta * S.rho_first, z2 = ta * S.rho_last, z3 = tb * S.rho_first, z4 = tb * S.rho_last;
-    const double zmin = S.s_z + fmin(fmin(z1, z2), fmin(z3, z4));
-    const double zmax = S.s_z + fmax(fmax(z1, z2), fmax(z3, z4));
-    const bool finite = (zmin > -1.0e9) && (zmax < 1.0e9);
-    int z0 = finite ? (((int)floor(zmin) - 1) & ~3) : 0;
+    const int i0 = C.i_start + C.dir * (b * kAlSB);
+    const int i = i0 + C.dir * s;
+    // z range of this line over the block's rows: p_z = s_z + t * r_z is monotone in the row
+    const double t0 = __dmul_rn(__dsub_rn((double)i0, C.s_m), C.inv_rm);
+    const double t = __dmul_rn(__dsub_rn((double)i, C.s_m), C.inv_rm);
+    const double za = S.s_z + t * S.rho_first, zb = S.s_z + t * S.rho_last;
+    const int zlo = __reduce_min_sync(0xffffffffu, al_to_int(floor(fmin(za, zb))));
+    const int zhi = __reduce_max_sync(0xffffffffu, al_to_int(floor(fmax(za, zb))));
     // taps k, k+1 with k = floor(p_z - z0) in [1, W-3] (one spare on either side for fp32 rounding)
-    const bool winok = finite && ((int)floor(zmax) + 3 - z0 <= W);
-    const bool live = winok && (i <= C.i_hi);
-    if (!winok && i <= C.i_hi) atomicOr(P.err_flag, 1u);
+    const int z0 = (zlo - 1) & ~3;
+    const int need = zhi + 3 - z0;
+    const bool winok = (zlo > -1000000000) && (zhi < 1000000000) && (need <= W);
+    const bool live = winok && (i >= C.i_lo) && (i <= C.i_hi);
     AlLine L;
     L.pa = L.pb = P.vol;
     L.u1 = 0.0f;
-    int flags = 0;
+    L.flags = 0;
     if (live) {
         const double ps = p_of_i(C.s_s, C.s_m, C.rt_s, i);           // Eq. 6 along the slow axis
         const double jf = floor(ps);
         const int j = (int)jf;
         L.u1 = ceil_weight<INTERP>((float)(ps - jf));
-        if (j >= 0 && j < C.n_s) flags |= 1;
-        if (j + 1 >= 0 && j + 1 < C.n_s) flags |= 2;
+        if (j >= 0 && j < C.n_s) L.flags |= 1;
+        if (j + 1 >= 0 && j + 1 < C.n_s) L.flags |= 2;
         L.pa = P.vol + ((long long)i * C.stride_m + (long long)j * C.stride_s);
         L.pb = L.pa + C.stride_s;
     }
-    L.z0f = (winok ? z0 : 0) | flags;
     L.pad_[0] = L.pad_[1] = 0;
     S.line[buf][l] = L;
-    if (s == 0) {
+    // a window that does not fit is never sampled out of bounds: park every row at p = 4
+    if (s == 0) S.t0[buf][c] = winok ? t0 : 0.0;
+    if (l == 0) {
+        if (!winok) atomicOr(P.err_flag, 1u);
         AlBatch B;
-        // a window that does not fit is never sampled out of bounds: park every row at p = 4
-        B.t0 = winok ? ta : 0.0;
         B.off = winok ? S.s_z - (double)z0 : 4.0;
-        S.batch[buf][c] = B;
+        B.z0 = winok ? z0 : 0;
+        B.nq = winok ? (need + 3) >> 2 : 0;
+        S.batch[buf] = B;
     }
 }
 
@@ -137,12 +149,13 @@ __device__ __forceinline__ void al_line_params(AlShared &S, const AlignedParams 
 // of kAlSB slices; per batch
 //   phase A: for each (column, slice) blend the two volume rows j, j+1 (float4 loads along z,
 //            zero-filled outside the volume) with the column's slow-axis weight and store the
-//            W-voxel window of the blended line in shared memory;
+//            needed part of the W-voxel window of the blended line in shared memory;
 //   phase B: every thread takes its row's sample from each staged line: position by one FMA
 //            from a per-(column, batch) fp64 anchor, floor by a round-down add of 2^23, two
-//            shared-memory taps, one lerp, one add (Alg. 1 l.7-18).
-// Line parameters of batch b+1 are computed by warp 0 during phase A of batch b (double
-// buffered), so a batch costs two block barriers.
+//            shared-memory taps, one lerp, one add (Alg. 1 l.7-18), two
+//            slices at a time in packed fp32x2 arithmetic (sm_100 FFMA2 / FADD2).
+// Parameters of batch b+1 are computed by warp 0 during phase A of batch b (double buffered),
+// so a batch costs two block barriers.
 // ------------------------------------------------------------------------------------------
 template <int INTERP, int W>
 __global__ void __launch_bounds__(kAlTV, 3)
@@ -159,10 +172,11 @@ fp_aligned_kernel(const __grid_constant__ AlignedParams P)
     const int row0 = blockIdx.y * kAlTV;
     const int iv = min(row0 + tid, P.nv - 1);
 
-    // ---- column set-up (Eqs. 1-5, Alg. 1 l.1-5), one thread per column
+    // ---- column set-up (Eqs. 1-5, Alg. 1 l.1-5), one thread per column; columns past the detector
+    //      edge reuse the last column's geometry with an empty slice range
     if (tid < kAlTU) {
         AlColumn C;
-        const int iu = iu0 + tid;
+        const int iu = min(iu0 + tid, P.nu - 1);
         double s[3], r[2];
 #pragma unroll
         for (int a = 0; a < 3; ++a) s[a] = __ddiv_rn(__dsub_rn(g[a], P.G.origin[a]), P.G.delta);
@@ -178,19 +192,17 @@ fp_aligned_kernel(const __grid_constant__ AlignedParams P)
         C.m = m;
         C.s_m = m ? s[1] : s[0];
         C.s_s = m ? s[0] : s[1];
-        C.rt_s = __ddiv_rn(m ? r[0] : r[1], rm);                  // Eq. 4
-        C.inv_rm = 1.0 / rm;
+        C.rt_s = rm != 0.0 ? __ddiv_rn(m ? r[0] : r[1], rm) : 0.0;   // Eq. 4
+        C.inv_rm = rm != 0.0 ? 1.0 / rm : 0.0;
         C.stride_m = m ? nz : ny * nz;
         C.stride_s = m ? ny * nz : nz;
         C.n_s = m ? P.G.n[0] : P.G.n[1];
         int lo = 0, hi = (m ? P.G.n[1] : P.G.n[0]) - 1;
-        if (iu < P.nu && rm != 0.0)
+        if (iu0 + tid < P.nu && rm != 0.0)
             clip_axis(C.s_s, C.s_m, C.rt_s, C.n_s, lo, hi);
-        else {
+        else
             hi = -1;
-            C.inv_rm = 0.0;
-            C.rt_s = 0.0;
-        }
+        if (lo > hi) { lo = 0; hi = -1; }
         C.i_lo = lo;
         C.i_hi = hi;
         S.col[tid] = C;
@@ -198,78 +210,125 @@ fp_aligned_kernel(const __grid_constant__ AlignedParams P)
             S.s_z = s[2];
             S.rho_first = al_rho(g, P.G, row0, s[2]);
             S.rho_last = al_rho(g, P.G, min(row0 + kAlTV, P.nv) - 1, s[2]);
+            S.lines_bias = (unsigned)__cvta_generic_to_shared(lines) - (0x4B000000u << 2);
         }
+    }
+    __syncthreads();
+    // common start: the smallest ray parameter t = (i_lo - s_m) / r_m among the block's columns; every
+    // column starts at the slice where its own t reaches it, so that the columns advance through the
+    // volume together and one z window serves the whole batch (matters where the driving axis switches
+    // inside the block and where neighbouring columns enter through a side face)
+    if (tid < kAlTU) {
+        double t_ref = 1.0e300;
+#pragma unroll
+        for (int c = 0; c < kAlTU; ++c) {
+            const AlColumn &C = S.col[c];
+            const int i_first = C.inv_rm < 0.0 ? C.i_hi : C.i_lo;
+            if (C.i_hi >= C.i_lo) t_ref = fmin(t_ref, ((double)i_first - C.s_m) * C.inv_rm);
+        }
+        AlColumn &C = S.col[tid];
+        const int dir = C.inv_rm < 0.0 ? -1 : 1;
+        int i_start = dir > 0 ? C.i_lo : C.i_hi;
+        if (t_ref < 1.0e299 && C.inv_rm != 0.0) {
+            // slice of this column at t_ref, never inside its own range; a column without slices just
+            // follows the others (its lines are never live)
+            const double x = C.s_m + t_ref / C.inv_rm;
+            if (C.i_hi < C.i_lo)
+                i_start = min(max(al_to_int(floor(x)), -65536), 65536 + C.n_s);
+            else if (dir > 0)
+                i_start = min(C.i_lo, max(al_to_int(floor(x)), C.i_lo - 65536));
+            else
+                i_start = max(C.i_hi, min(al_to_int(ceil(x)), C.i_hi + 65536));
+        }
+        C.i_start = i_start;
+        C.dir = dir;
     }
     __syncthreads();
     if (tid == 0) {
         int nb = 0;
 #pragma unroll
-        for (int c = 0; c < kAlTU; ++c) nb = max(nb, (S.col[c].i_hi - S.col[c].i_lo + 1 + kAlSB - 1) / kAlSB);
+        for (int c = 0; c < kAlTU; ++c) {
+            const AlColumn &C = S.col[c];
+            if (C.i_hi >= C.i_lo) nb = max(nb, ((C.dir > 0 ? C.i_hi - C.i_start : C.i_start - C.i_lo) + kAlSB) / kAlSB);
+        }
         S.n_batches = nb;
-        S.lines_bias = (unsigned)__cvta_generic_to_shared(lines) - (0x4B000000u << 2);
     }
-    if (tid < kAlNL) al_line_params<INTERP, W>(S, P, 0, 0, tid);
+    __syncthreads();
+    if (tid < kAlNL) al_batch_params<INTERP, W>(S, P, 0, 0, tid);
 
     // ---- per-thread constants: r_z of this row, per-column z increment per slice
-    const double s_z = S.s_z;
-    const double rho = al_rho(g, P.G, iv, s_z);
-    float dz[kAlTU], acc[kAlTU];
+    const double rho = al_rho(g, P.G, iv, S.s_z);
+    float dz[kAlTU];
+    float2 acc[kAlTU];
 #pragma unroll
     for (int c = 0; c < kAlTU; ++c) {
-        dz[c] = (float)(rho * S.col[c].inv_rm);
-        acc[c] = 0.0f;
+        dz[c] = (float)(rho * S.col[c].inv_rm * (double)S.col[c].dir);
+        acc[c] = make_float2(0.0f, 0.0f);
     }
     __syncthreads();
     const int n_batches = S.n_batches;
-    const int nz = P.G.n[2];
-    const int warp = tid >> 5, lane = tid & 31;
-    constexpr int QW = W / 4;
-    constexpr int kWarps = kAlTV / 32;
-    // shared-memory byte address of lines[0] minus the bias the 2^23 trick leaves in the float's bits
     // read back from shared memory so that neither compiler can split the bias into address + constant:
     // (bits << 2) + bias stays ONE add and the per-line constant folds into the load's immediate offset
     const unsigned lines_bias = *reinterpret_cast<volatile unsigned *>(&S.lines_bias);
-    constexpr float kMagic = 8388608.0f;      // 2^23: x + 2^23 rounded down = floor(x) for 0 <= x < 2^22
+    const int nz = P.G.n[2];
+    const int warp = tid >> 5, lane = tid & 31;
+    constexpr int kWarps = kAlTV / 32;
+    const float2 kMagic2 = make_float2(8388608.0f, 8388608.0f);      // 2^23
+    const float2 kNegMagic2 = make_float2(-8388608.0f, -8388608.0f);
+    const float2 kNegOne2 = make_float2(-1.0f, -1.0f);
 
     for (int b = 0; b < n_batches; ++b) {
         const int buf = b & 1;
         if (b) __syncthreads();               // parameters of batch b visible, phase B of b-1 done
+        const AlBatch B = S.batch[buf];
         // ---------------- phase A
 #pragma unroll
         for (int l = warp; l < kAlNL; l += kWarps) {
             const AlLine L = S.line[buf][l];
-            const int z0 = L.z0f & ~3;
+            const float2 u2 = make_float2(L.u1, L.u1);
             float4 *dst = reinterpret_cast<float4 *>(lines + l * W);
+            // all loads of the line first (predicated, no branches: they overlap), then the blends
+            float4 va[W / 128], vb[W / 128];
 #pragma unroll
-            for (int q = lane; q < QW; q += 32) {
-                const int z = z0 + 4 * q;
-                const bool inz = (unsigned)z < (unsigned)nz;
-                float4 va = make_float4(0.f, 0.f, 0.f, 0.f), vb = va;
-                if (inz && (L.z0f & 1)) va = __ldg(reinterpret_cast<const float4 *>(L.pa + z));
-                if (inz && (L.z0f & 2)) vb = __ldg(reinterpret_cast<const float4 *>(L.pb + z));
-                float4 o;
-                o.x = fmaf(L.u1, vb.x - va.x, va.x);
-                o.y = fmaf(L.u1, vb.y - va.y, va.y);
-                o.z = fmaf(L.u1, vb.z - va.z, va.z);
-                o.w = fmaf(L.u1, vb.w - va.w, va.w);
-                dst[q] = o;
+            for (int k = 0; k < W / 128; ++k) {
+                const int q = lane + 32 * k;
+                const int z = B.z0 + 4 * q;
+                const bool ok = (q < B.nq) && ((unsigned)z < (unsigned)nz);
+                va[k] = make_float4(0.f, 0.f, 0.f, 0.f);
+                vb[k] = va[k];
+                if (ok && (L.flags & 1)) va[k] = __ldg(reinterpret_cast<const float4 *>(L.pa + z));
+                if (ok && (L.flags & 2)) vb[k] = __ldg(reinterpret_cast<const float4 *>(L.pb + z));
+            }
+#pragma unroll
+            for (int k = 0; k < W / 128; ++k) {
+                const int q = lane + 32 * k;
+                // va + u (vb - va), two voxels per instruction
+                const float2 d0 = __ffma2_rn(make_float2(va[k].x, va[k].y), kNegOne2, make_float2(vb[k].x, vb[k].y));
+                const float2 d1 = __ffma2_rn(make_float2(va[k].z, va[k].w), kNegOne2, make_float2(vb[k].z, vb[k].w));
+                const float2 o0 = __ffma2_rn(u2, d0, make_float2(va[k].x, va[k].y));
+                const float2 o1 = __ffma2_rn(u2, d1, make_float2(va[k].z, va[k].w));
+                if (q < B.nq) dst[q] = make_float4(o0.x, o0.y, o1.x, o1.y);
             }
         }
-        if (tid < kAlNL && b + 1 < n_batches) al_line_params<INTERP, W>(S, P, buf ^ 1, b + 1, tid);
+        if (tid < kAlNL && b + 1 < n_batches) al_batch_params<INTERP, W>(S, P, buf ^ 1, b + 1, tid);
         __syncthreads();
         // ---------------- phase B
 #pragma unroll
         for (int c = 0; c < kAlTU; ++c) {
-            const AlBatch B = S.batch[buf][c];
-            const float a = (float)fma(B.t0, rho, B.off);
+            const float a = (float)fma(S.t0[buf][c], rho, B.off);
 #pragma unroll
-            for (int s = 0; s < kAlSB; ++s) {
-                const float p = fmaf((float)s, dz[c], a);
-                const float x = __fadd_rd(p, kMagic);             // bits = 0x4B000000 + floor(p)
-                const float d = p - (x - kMagic);
-                const unsigned addr = (__float_as_uint(x) << 2) + lines_bias + (unsigned)((c * kAlSB + s) * W * 4);
-                const float v0 = al_lds(addr), v1 = al_lds(addr + 4u);
-                acc[c] += fmaf(ceil_weight<INTERP>(d), v1 - v0, v0);
+            for (int s = 0; s < kAlSB; s += 2) {
+                const float2 p = __ffma2_rn(make_float2((float)s, (float)(s + 1)), make_float2(dz[c], dz[c]), make_float2(a, a));
+                const float2 x = __fadd2_rd(p, kMagic2);                  // bits = 0x4B000000 + floor(p)
+                const float2 f = __fadd2_rn(x, kNegMagic2);
+                const float2 d = __ffma2_rn(f, kNegOne2, p);              // p - floor(p)
+                const unsigned a0 = (__float_as_uint(x.x) << 2) + lines_bias + (unsigned)((c * kAlSB + s) * W * 4);
+                const unsigned a1 = (__float_as_uint(x.y) << 2) + lines_bias + (unsigned)((c * kAlSB + s + 1) * W * 4);
+                const float2 v0 = make_float2(al_lds(a0), al_lds(a1));
+                const float2 v1 = make_float2(al_lds(a0 + 4u), al_lds(a1 + 4u));
+                const float2 wz = make_float2(ceil_weight<INTERP>(d.x), ceil_weight<INTERP>(d.y));
+                const float2 df = __ffma2_rn(v0, kNegOne2, v1);           // v1 - v0
+                acc[c] = __fadd2_rn(acc[c], __ffma2_rn(wz, df, v0));
             }
         }
     }
@@ -285,7 +344,7 @@ fp_aligned_kernel(const __grid_constant__ AlignedParams P)
             // same summation order as the definition: x^2 + y^2 + z^2 with r~_m = 1
             const double a0 = S.col[c].m ? rs * rs : 1.0, a1 = S.col[c].m ? 1.0 : rs * rs;
             const double L = sqrt((a0 + a1) + rz * rz);
-            o[c] = (float)(P.G.delta * L) * acc[c];
+            o[c] = (float)(P.G.delta * L) * (acc[c].x + acc[c].y);
         }
         float *dst = P.out + ((size_t)proj * P.nv + iv) * P.nu + iu0;
         if ((P.nu & 3) == 0 && iu0 + kAlTU <= P.nu) {
