@@ -103,7 +103,8 @@ def oracle_sample(cfg, geom, vol_np, max_seconds=20.0):
     ids, values, mfl, pathlen, margins)."""
     import oracle
     cores = oracle.host_cores()
-    projs = [0, cfg.n_proj // 8]
+    # eight poses spread over the orbit: both driving axes, both signs, and the switches between them
+    projs = sorted({(k * cfg.n_proj) // 8 + (cfg.n_proj // 16 if k % 2 else 0) for k in range(8)})
     # calibrate on a few rows, then size the sample for ~max_seconds of wall time
     rows_cal = max(1, min(cfg.nv, 4))
     def ids_for(rows):
@@ -122,8 +123,8 @@ def oracle_sample(cfg, geom, vol_np, max_seconds=20.0):
     n_samples = int(np.maximum(mfl[:, 2] - mfl[:, 1] + 1, 0).sum())
     rays_per_proj = cfg.nu * cfg.nv
     proj_per_s = (len(ids) / rays_per_proj) / dt
-    desc = "%d of %d detector rows (all %d columns) of projections %s: %d rays, %d samples in %.1f s" % (
-        rows, cfg.nv, cfg.nu, projs, len(ids), n_samples, dt)
+    desc = "%d of %d detector rows (all %d columns) of %d projections %s: %d rays, %d samples in %.1f s" % (
+        rows, cfg.nv, cfg.nu, len(projs), projs, len(ids), n_samples, dt)
     return proj_per_s, n_samples / dt, cores, desc, ids, val, mfl, pl, mg
 
 
@@ -156,6 +157,22 @@ def run_reference(args):
     }
     print(json.dumps(line))
     return 0
+
+
+def max_over_ranks(dist, value, device="cuda"):
+    """MAX of a python float over all ranks (identity without a process group)."""
+    if dist is None:
+        return float(value)
+    import torch
+    t = torch.tensor([float(value)], device=device, dtype=torch.float64)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def replicas_throughput(world, units_per_rank, seconds_max):
+    """Whole-job rate of `world` independent replicas: every rank processes the
+    same number of units, the job takes as long as its slowest rank."""
+    return world * units_per_rank / seconds_max
 
 
 def workload_name(cfg):
@@ -242,13 +259,10 @@ def main():
     clk = clocks.stop()
     step_ms = [ev[k].elapsed_time(ev[k + 1]) for k in range(args.steps)]
     total_ms = ev[0].elapsed_time(ev[args.steps])
-    t = torch.tensor([total_ms], device="cuda", dtype=torch.float64)
-    if dist is not None:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    total_ms = float(t.item())
+    total_ms = max_over_ranks(dist, total_ms)
     ms_per_step = total_ms / args.steps
-    proj_per_s = world * cfg.n_proj / (ms_per_step * 1e-3)
-    samples_per_s = world * samples / (ms_per_step * 1e-3)
+    proj_per_s = replicas_throughput(world, cfg.n_proj, ms_per_step * 1e-3)
+    samples_per_s = replicas_throughput(world, samples, ms_per_step * 1e-3)
 
     # ---- end to end through fp_project_host: pinned host volume in, pinned host projections out
     e2e = None
@@ -264,11 +278,8 @@ def main():
         for _ in range(n_e2e):
             P2.project_host(vol_h, geom, cfg.nu, cfg.nv, out_host=out_h)      # synchronises before returning
         dt = time.perf_counter() - t0
-        t = torch.tensor([dt], device="cuda", dtype=torch.float64)
-        if dist is not None:
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        dt = float(t.item())
-        e2e = {"value": world * cfg.n_proj * n_e2e / dt, "unit": UNIT,
+        dt = max_over_ranks(dist, dt)
+        e2e = {"value": replicas_throughput(world, cfg.n_proj * n_e2e, dt), "unit": UNIT,
                "h2d_bytes_per_step": int(vol_h.numel() * 4 + geom.size * 8),
                "d2h_bytes_per_step": int(out_h.numel() * 4), "steps": n_e2e,
                "same_result_as_device_path": bool(torch.equal(out_h, out.cpu()))}

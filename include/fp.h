@@ -146,6 +146,16 @@ fp_status fp_ray_ranges(fp_ctx *ctx, int n_proj, const double *geom_host, int nu
  */
 fp_status fp_last_sample_count(fp_ctx *ctx, unsigned long long *n);
 
+/*
+ * fp_plan: the host-side plan fp_project makes for ONE pose (no device needed, nothing is launched):
+ *   *kernel    FP_KERNEL_ALIGNED or FP_KERNEL_DIRECT: the sampling kernel FP_KERNEL_AUTO picks
+ *   *window    staging window of the aligned kernel in voxels along z (0 for the direct kernel)
+ *   *z_driven  1 if some ray of the pose has z as its driving axis (Eq. 2), which is
+ *              what makes fp_project build the permuted copy of the layout stage
+ * Assumes a 16-byte aligned volume pointer.  geom_host: host, double [12].
+ */
+fp_status fp_plan(fp_ctx *ctx, const double *geom_host, int nu, int nv, int *kernel, int *window, int *z_driven);
+
 /* fp_last_launch_count: how many kernels of this library the most recent fp_project enqueued. */
 fp_status fp_last_launch_count(fp_ctx *ctx, int *n);
 

@@ -518,6 +518,18 @@ extern "C" fp_status fp_last_sample_count(fp_ctx *c, unsigned long long *n)
     return FP_OK;
 }
 
+extern "C" fp_status fp_plan(fp_ctx *c, const double *geom, int nu, int nv, int *kernel, int *window, int *z_driven)
+{
+    if (!c || !geom || !kernel || !window || !z_driven) return fail(c, FP_ERR_INVALID_ARG, "fp_plan: null argument");
+    if (nu < 1 || nv < 1) return fail(c, FP_ERR_INVALID_ARG, "nu, nv must be >= 1");
+    const int w = c->opt_kernel == FP_KERNEL_DIRECT ? 0 : plan_aligned(c, nullptr, geom, nu, nv);
+    const bool al = w > 0 && w <= kAlignedMaxW;
+    *kernel = al ? FP_KERNEL_ALIGNED : FP_KERNEL_DIRECT;
+    *window = al ? w : 0;
+    *z_driven = has_z_driven(geom, nu, nv) ? 1 : 0;
+    return FP_OK;
+}
+
 extern "C" fp_status fp_last_launch_count(fp_ctx *c, int *n)
 {
     if (!c || !n) return FP_ERR_INVALID_ARG;

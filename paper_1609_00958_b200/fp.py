@@ -24,7 +24,7 @@ INTERP_LINEAR, INTERP_SPLINE = 0, 1
 
 # every symbol include/fp.h declares (tests check the library exports all of them)
 SYMBOLS = ["fp_create", "fp_destroy", "fp_set_option", "fp_get_option", "fp_prepare", "fp_project",
-           "fp_project_host", "fp_ray_ranges", "fp_last_sample_count", "fp_last_launch_count",
+           "fp_project_host", "fp_ray_ranges", "fp_plan", "fp_last_sample_count", "fp_last_launch_count",
            "fp_status_string", "fp_last_error", "fp_version"]
 
 
@@ -61,10 +61,11 @@ def load(build_if_missing: bool = True):
     L.fp_project.argtypes = [vp, vp, i, dp, i, i, vp, vp]
     L.fp_project_host.argtypes = [vp, vp, i, dp, i, i, vp]
     L.fp_ray_ranges.argtypes = [vp, i, dp, i, i, vp, vp]
+    L.fp_plan.argtypes = [vp, dp, i, i, ctypes.POINTER(i), ctypes.POINTER(i), ctypes.POINTER(i)]
     L.fp_last_sample_count.argtypes = [vp, ctypes.POINTER(ctypes.c_ulonglong)]
     L.fp_last_launch_count.argtypes = [vp, ctypes.POINTER(i)]
     for name in ("fp_create", "fp_destroy", "fp_set_option", "fp_get_option", "fp_prepare", "fp_project",
-                 "fp_project_host", "fp_ray_ranges", "fp_last_sample_count", "fp_last_launch_count"):
+                 "fp_project_host", "fp_ray_ranges", "fp_plan", "fp_last_sample_count", "fp_last_launch_count"):
         getattr(L, name).restype = i
     L.fp_status_string.argtypes = [i]
     L.fp_status_string.restype = ctypes.c_char_p
@@ -190,6 +191,14 @@ class Projector:
         self._check(self._L.fp_ray_ranges(self._h, n_proj, g.ctypes.data_as(ctypes.POINTER(ctypes.c_double)),
                                           int(nu), int(nv), mfl.data_ptr(), _stream_handle(stream)))
         return mfl
+
+    def plan(self, geom_row, nu: int, nv: int):
+        """fp_plan: (kernel, window, z_driven) the library would use for one pose; host only."""
+        g = np.ascontiguousarray(geom_row, dtype=np.float64).reshape(12)
+        k, w, z = ctypes.c_int(), ctypes.c_int(), ctypes.c_int()
+        self._check(self._L.fp_plan(self._h, g.ctypes.data_as(ctypes.POINTER(ctypes.c_double)), int(nu), int(nv),
+                                    ctypes.byref(k), ctypes.byref(w), ctypes.byref(z)))
+        return k.value, w.value, bool(z.value)
 
     def last_sample_count(self) -> int:
         n = ctypes.c_ulonglong()
