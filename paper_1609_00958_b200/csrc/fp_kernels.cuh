@@ -62,10 +62,90 @@ __device__ __forceinline__ void block_count_samples(unsigned long long *counter,
 
 // ------------------------------------------------------------------------------------------
 // Direct sampling kernel: one thread per ray, taps read straight from global memory through
-// the read-only path, index-masked (zero-extended volume, reading #2).
-// Alg. 1 lines 6-20; Eq. 6 (:104) in the multiply form anchored at the
-// middle slice of the ray; Eq. 15 (:165) tap selection; Eq. 11 (:142) product weights.
+// the read-only path.  Alg. 1 lines 6-20; Eq. 6 (:104) in the multiply form;
+// Eq. 15 (:165) tap selection; Eq. 11 (:142) product weights.
+//
+// Eq. 6 is evaluated in fp32 per segment of kSegment slices: the anchor p_t(i_c) of the segment's
+// middle slice comes from fp64 and is split into an integer voxel index and a fraction in [0,1),
+// so |fp32 operand| <= kSegment/2 + 1 whatever the volume size.  Both transverse
+// coordinates travel as one packed fp32x2 value (sm_100 FFMA2 / FADD2); floor is a round-down add
+// of 1.5 * 2^23, whose low mantissa bits are the integer part.
+//
+// A ray's slices are split into an interior run, where all four taps of every sample are inside
+// the volume (0.5 <= p_t <= N_t - 1.5 in fp64, far more margin than the fp32 error), sampled
+// without masks, and the two edge runs before and after it, where taps are masked by index
+// (zero-extended volume, reading #2).
 // ------------------------------------------------------------------------------------------
+template <int INTERP, bool MASKED>
+__device__ __forceinline__ float direct_run(const RaySetup &R, const AxisLayout &A, int lo, int hi)
+{
+    float acc = 0.0f;
+    const float2 r2 = make_float2((float)R.rt_a, (float)R.rt_b);
+    const float *__restrict__ base = A.base;
+    const long long si = A.si, ss = A.ss, sf = A.sf;
+    const unsigned n_s = (unsigned)A.n_s, n_f = (unsigned)A.n_f;
+    const float2 kMagic2 = make_float2(12582912.0f, 12582912.0f), kNegMagic2 = make_float2(-12582912.0f, -12582912.0f);
+    const float2 kNegOne2 = make_float2(-1.0f, -1.0f), kOne2 = make_float2(1.0f, 1.0f);
+    for (int s0 = lo; s0 <= hi; s0 += kSegment) {
+        const int s1 = min(s0 + kSegment - 1, hi);
+        const int ic = (s0 + s1) >> 1;
+        const double pa = p_of_i(R.s_a, R.s_m, R.rt_a, ic), pb = p_of_i(R.s_b, R.s_m, R.rt_b, ic);
+        const double fa = floor(pa), fb = floor(pb);
+        const int ja = (int)fa, kb = (int)fb;
+        const float2 a2 = make_float2((float)(pa - fa), (float)(pb - fb));
+        const float *qseg = base + (long long)ja * ss + (long long)kb * sf + (long long)s0 * si;
+        float2 fi = make_float2((float)(s0 - ic), (float)(s0 - ic));
+        for (int i = s0; i <= s1; ++i) {
+            const float2 p = __ffma2_rn(fi, r2, a2);
+            fi = __fadd2_rn(fi, kOne2);
+            const float2 x = __fadd2_rd(p, kMagic2);              // bits = 0x4B400000 + floor(p)
+            const float2 d = __ffma2_rn(__fadd2_rn(x, kNegMagic2), kNegOne2, p);
+            const int jl = __float_as_int(x.x) - 0x4B400000, kl = __float_as_int(x.y) - 0x4B400000;
+            const float u1 = ceil_weight<INTERP>(d.x), u2 = ceil_weight<INTERP>(d.y);
+            const float *q = qseg + (long long)jl * ss + (long long)kl * sf;
+            qseg += si;
+            float v00, v01, v10, v11;
+            if (MASKED) {
+                const int j = ja + jl, k = kb + kl;
+                const bool j0 = (unsigned)j < n_s, j1 = (unsigned)(j + 1) < n_s;
+                const bool k0 = (unsigned)k < n_f, k1 = (unsigned)(k + 1) < n_f;
+                v00 = (j0 && k0) ? __ldg(q) : 0.0f;
+                v01 = (j0 && k1) ? __ldg(q + sf) : 0.0f;
+                v10 = (j1 && k0) ? __ldg(q + ss) : 0.0f;
+                v11 = (j1 && k1) ? __ldg(q + ss + sf) : 0.0f;
+            } else {
+                v00 = __ldg(q);
+                v01 = __ldg(q + sf);
+                v10 = __ldg(q + ss);
+                v11 = __ldg(q + ss + sf);
+            }
+            // lerp along the fast axis for both rows at once, then along the slow axis
+            const float2 lo2 = make_float2(v00, v10);
+            const float2 t = __ffma2_rn(make_float2(u2, u2), __ffma2_rn(lo2, kNegOne2, make_float2(v01, v11)), lo2);
+            acc += fmaf(u1, t.y - t.x, t.x);
+        }
+    }
+    return acc;
+}
+
+// Slices of [lo, hi] on which lo_p <= s_t + (i - s_m) rt <= hi_p (fp64, one slice of slack inwards).
+__device__ __forceinline__ void interior_clip(double s_t, double s_m, double rt, double lo_p, double hi_p, int &lo, int &hi)
+{
+    if (!(lo_p <= hi_p)) {            // fewer than two voxels along this axis: no interior
+        hi = lo - 1;
+        return;
+    }
+    if (rt == 0.0) {
+        if (!(s_t >= lo_p && s_t <= hi_p)) hi = lo - 1;
+        return;
+    }
+    const double x1 = s_m + (lo_p - s_t) / rt, x2 = s_m + (hi_p - s_t) / rt;
+    const int a = clamp_to_int(ceil(fmin(x1, x2)) + 1.0, lo, hi + 1);
+    const int b = clamp_to_int(floor(fmax(x1, x2)) - 1.0, lo - 1, hi);
+    lo = max(lo, a);
+    hi = min(hi, b);
+}
+
 template <int INTERP>
 __global__ void __launch_bounds__(kDirectThreads)
 fp_direct_kernel(const __grid_constant__ ProjectParams P)
@@ -91,40 +171,16 @@ fp_direct_kernel(const __grid_constant__ ProjectParams P)
         if (R.i_last >= R.i_first) {
             n_samples = R.i_last - R.i_first + 1;
             const AxisLayout &A = P.lay[R.m];
-            const float r1 = (float)R.rt_a, r2 = (float)R.rt_b;
-            const float *__restrict__ base = A.base;
-            const long long si = A.si, ss = A.ss, sf = A.sf;
-            const unsigned n_s = (unsigned)A.n_s, n_f = (unsigned)A.n_f;
-            // Eq. 6 evaluated in fp32 per segment of kSegment slices: the anchor p_t(i_c) of the
-            // segment's middle slice comes from fp64 and is split into an integer voxel index
-            // and a fraction in [0,1), so |fp32 operand| <= kSegment/2 + 1 whatever the volume
-            // size.
-            for (int s0 = R.i_first; s0 <= R.i_last; s0 += kSegment) {
-                const int s1 = min(s0 + kSegment - 1, R.i_last);
-                const int ic = (s0 + s1) >> 1;
-                const double pa = p_of_i(R.s_a, R.s_m, R.rt_a, ic), pb = p_of_i(R.s_b, R.s_m, R.rt_b, ic);
-                const double fa = floor(pa), fb = floor(pb);
-                const int ja = (int)fa, kb = (int)fb;
-                const float a1 = (float)(pa - fa), a2 = (float)(pb - fb);
-                const float *qseg = base + (long long)ja * ss + (long long)kb * sf;
-                for (int i = s0; i <= s1; ++i) {
-                    const float fi = (float)(i - ic);
-                    const float p1 = fmaf(fi, r1, a1), p2 = fmaf(fi, r2, a2);
-                    const float f1 = floorf(p1), f2 = floorf(p2);
-                    const int jl = (int)f1, kl = (int)f2;
-                    const int j = ja + jl, k = kb + kl;
-                    const float u1 = ceil_weight<INTERP>(p1 - f1), u2 = ceil_weight<INTERP>(p2 - f2);
-                    const bool j0 = (unsigned)j < n_s, j1 = (unsigned)(j + 1) < n_s;
-                    const bool k0 = (unsigned)k < n_f, k1 = (unsigned)(k + 1) < n_f;
-                    const float *q = qseg + (long long)i * si + (long long)jl * ss + (long long)kl * sf;
-                    const float v00 = (j0 && k0) ? __ldg(q) : 0.0f;
-                    const float v01 = (j0 && k1) ? __ldg(q + sf) : 0.0f;
-                    const float v10 = (j1 && k0) ? __ldg(q + ss) : 0.0f;
-                    const float v11 = (j1 && k1) ? __ldg(q + ss + sf) : 0.0f;
-                    const float t0 = fmaf(u2, v01 - v00, v00);
-                    const float t1 = fmaf(u2, v11 - v10, v10);
-                    acc += fmaf(u1, t1 - t0, t0);
-                }
+            // interior run: every tap of every sample inside the volume
+            int in_lo = R.i_first, in_hi = R.i_last;
+            interior_clip(R.s_a, R.s_m, R.rt_a, 0.5, (double)A.n_s - 1.5, in_lo, in_hi);
+            if (in_lo <= in_hi) interior_clip(R.s_b, R.s_m, R.rt_b, 0.5, (double)A.n_f - 1.5, in_lo, in_hi);
+            if (in_lo <= in_hi) {
+                acc = direct_run<INTERP, true>(R, A, R.i_first, in_lo - 1);
+                acc += direct_run<INTERP, false>(R, A, in_lo, in_hi);
+                acc += direct_run<INTERP, true>(R, A, in_hi + 1, R.i_last);
+            } else {
+                acc = direct_run<INTERP, true>(R, A, R.i_first, R.i_last);
             }
         }
         const float scale = (float)(P.G.delta * R.L);       // step length

@@ -87,6 +87,22 @@ def test_c2_128_cube_full_orbit(torch, fp, synth, oracle):
     assert n == int(np.maximum(mfl[..., 2] - mfl[..., 1] + 1, 0).sum())
 
 
+def test_c1_and_c2_through_the_direct_kernel(torch, fp, synth, oracle):
+    """FP_OPT_KERNEL = FP_KERNEL_DIRECT: the general-pose kernel on the circular-orbit configs (the
+    default plan would pick the aligned kernel for all of them)."""
+    cfg = synth.CONFIGS["C1"]
+    worst, _, _ = compare_full(torch, fp, oracle, synth.make_volume(cfg).numpy(), cfg.voxel_size, cfg.origin,
+                               synth.make_geometry(cfg), cfg.nu, cfg.nv,
+                               options=[(fp.OPT_KERNEL, fp.KERNEL_DIRECT)], what="C1 direct")
+    assert worst < 1.0
+    cfg = synth.CONFIGS["C2"]
+    vol = synth.make_volume(cfg).numpy()
+    geom = synth.make_geometry(cfg)[[0, 22, 23, 45, 90, 113, 158]]
+    worst, _, _ = compare_full(torch, fp, oracle, vol, cfg.voxel_size, cfg.origin, geom, cfg.nu, cfg.nv,
+                               options=[(fp.OPT_KERNEL, fp.KERNEL_DIRECT)], what="C2 direct")
+    assert worst < 1.0
+
+
 def _big_config_subset(torch, fp, synth, oracle, name, projs, n_random, batch=None):
     """Full-size volume on the device, the launch configuration bench.py times (whole batches
     through fp_project), compared on sampled rays the oracle computes one by one."""
