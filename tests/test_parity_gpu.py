@@ -300,3 +300,64 @@ def test_reuse_context_changed_volume_and_streams(torch, fp, synth, oracle):
             ov, om, pl, mg = oracle.project_rays(v, delta, origin, geom, ids)
             gm = P.ray_ranges(geom, 32, 32).cpu().numpy()
             assert assert_parity(out.cpu().numpy().ravel(), gm.reshape(-1, 3), ov, om, pl, mg, float(np.abs(v).max())) < 1.0
+
+
+# ----------------------------------------------------------------------------- aligned kernel edge cases
+
+def aligned_pose(theta, sid, sdd, nu, nv, pitch, src_z=0.0, det_shift=(0.0, 0.0), flip_u=False, flip_v=False):
+    """v parallel to z, u perpendicular to z: the geometry class fp_aligned_kernel takes."""
+    c, s = math.cos(theta), math.sin(theta)
+    S = np.array([sid * c, sid * s, src_z])
+    C = S - sdd * np.array([c, s, 0.0])
+    U = pitch * np.array([-s, c, 0.0]) * (-1.0 if flip_u else 1.0)
+    V = pitch * np.array([0.0, 0.0, 1.0]) * (-1.0 if flip_v else 1.0)
+    O = C - ((nu - 1) / 2 + det_shift[0]) * U - ((nv - 1) / 2 + det_shift[1]) * V
+    return np.concatenate([S, O, U, V])
+
+
+@pytest.mark.parametrize("nu,nv,interp", [(37, 300, 0), (8, 5, 0), (66, 40, 1)])
+def test_aligned_kernel_edge_cases(torch, fp, oracle, nu, nv, interp):
+    """Ragged detectors (nu not a multiple of 8 or 4, more than one 256-row block), exact |r_x| = |r_y|
+    ties and the axis switch inside a block (45 degrees), both senses of u and v, a source off the
+    mid-plane, a detector shifted so far that some columns and rows miss, rays parallel to an axis."""
+    rng = np.random.default_rng(300 + nu)
+    shape = (21, 18, 24)                                    # nz a multiple of 4
+    vol = rng.uniform(-1.0, 2.0, size=shape).astype(np.float32)
+    delta = 0.8
+    origin = tuple(-(n - 1) / 2.0 * delta + 0.17 * k for k, n in enumerate(shape))
+    pitch = 0.9 * 24 * delta * 2.2 / nv if nv > 100 else 0.55
+    poses = []
+    for k, th in enumerate([0.0, math.pi / 4, 0.7853, 1.1, math.pi / 2, 2.5, math.pi, 3.9269908, 4.4, 5.9]):
+        poses.append(aligned_pose(th, 40.0, 90.0, nu, nv, pitch, src_z=(k % 3 - 1) * 3.0,
+                                  det_shift=((k % 4) * 2.5, -(k % 2) * 3.0), flip_u=bool(k & 1), flip_v=bool(k & 2)))
+    geom = np.stack(poses)
+    with fp.Projector(*shape, delta, origin) as P:
+        assert all(P.plan(g, nu, nv)[0] == fp.KERNEL_ALIGNED for g in geom)
+    worst, out, om = compare_full(torch, fp, oracle, vol, delta, origin, geom, nu, nv,
+                                  options=[(fp.OPT_INTERP, interp)], kernel=interp, what="aligned %dx%d" % (nu, nv))
+    assert worst < 1.0
+    assert set(np.unique(om[:, 0])) <= {0, 1}
+    if nv > 100:
+        assert (om[:, 2] < om[:, 1]).any() and (om[:, 2] >= om[:, 1]).any()     # some rays miss, most hit
+
+
+def test_aligned_kernel_window_sizes_and_direct_kernel_agree(torch, fp):
+    """The aligned kernel (whatever staging window the plan picks) and the direct kernel are two
+    implementations of the same sum: on the same inputs they agree to fp32 rounding (a property that
+    needs no oracle, so it runs at a size the oracle would not finish)."""
+    from paper_1609_00958_b200 import synth
+    cfg = synth.CONFIGS["C2"]
+    vol = synth.make_volume(cfg, device="cuda")
+    windows = set()
+    for pitch, nv in [(0.7, 64), (1.5, 192), (2.0, 256), (2.5, 270)]:
+        geom = np.stack([aligned_pose(th, cfg.sid, cfg.sdd, 96, nv, pitch) for th in (0.2, 0.8, 2.0, 4.0)])
+        with fp.Projector(*cfg.n, cfg.voxel_size, cfg.origin) as P:
+            plans = [P.plan(g, 96, nv) for g in geom]
+            assert all(k == fp.KERNEL_ALIGNED for k, _, _ in plans), plans
+            windows.add((max(w for _, w, _ in plans) + 127) // 128)
+            a = P.project(vol, geom, 96, nv).cpu().numpy().astype(np.float64)
+            P.set_option(fp.OPT_KERNEL, fp.KERNEL_DIRECT)
+            b = P.project(vol, geom, 96, nv).cpu().numpy().astype(np.float64)
+        scale = np.abs(b).max()
+        assert np.abs(a - b).max() <= 2e-5 * scale, (pitch, nv, np.abs(a - b).max(), scale)
+    assert len(windows) >= 3                                # several of the 128 / 256 / 384 / 512 instantiations ran
