@@ -67,7 +67,10 @@ enum {
      * whose u vector is perpendicular to it and that have no z-driven ray (every circular orbit
      * about z), FP_KERNEL_DIRECT (one thread per ray, four global taps per
      * sample) for every other pose.  FP_KERNEL_DIRECT forces the direct kernel for all poses;
-     * FP_KERNEL_ALIGNED behaves like AUTO (poses it cannot take still use the direct kernel). */
+     * FP_KERNEL_ALIGNED behaves like AUTO (poses it cannot take still use the direct kernel).
+     * FP_KERNEL_TMA: like AUTO, but calls whose aligned poses all fit a 256-voxel z window and 12 volume
+     * rows per block and slice are sampled by the TMA-fed kernel (tiles of the caller's volume copied to
+     * shared memory by cp.async.bulk.tensor, four taps per sample read from the tile). */
     FP_OPT_KERNEL = 1,
     /* 1 (default): the volume contents may have changed since the last call, internal copies
      * are rebuilt by every fp_project that needs them.  0: internal copies made by fp_prepare
@@ -85,7 +88,7 @@ enum {
     FP_OPT_COUNT_SAMPLES = 5
 };
 
-enum { FP_KERNEL_AUTO = 0, FP_KERNEL_DIRECT = 1, FP_KERNEL_ALIGNED = 2 };
+enum { FP_KERNEL_AUTO = 0, FP_KERNEL_DIRECT = 1, FP_KERNEL_ALIGNED = 2, FP_KERNEL_TMA = 3 };
 enum { FP_INTERP_LINEAR = 0, FP_INTERP_SPLINE = 1 };
 
 /*
@@ -148,7 +151,8 @@ fp_status fp_last_sample_count(fp_ctx *ctx, unsigned long long *n);
 
 /*
  * fp_plan: the host-side plan fp_project makes for ONE pose (no device needed, nothing is launched):
- *   *kernel    FP_KERNEL_ALIGNED or FP_KERNEL_DIRECT: the sampling kernel FP_KERNEL_AUTO picks
+ *   *kernel    FP_KERNEL_ALIGNED, FP_KERNEL_TMA or FP_KERNEL_DIRECT: the sampling kernel a call with this
+ *              pose alone would use under the current FP_OPT_KERNEL
  *   *window    staging window of the aligned kernel in voxels along z (0 for the direct kernel)
  *   *z_driven  1 if some ray of the pose has z as its driving axis (Eq. 2), which is
  *              what makes fp_project build the permuted copy of the layout stage

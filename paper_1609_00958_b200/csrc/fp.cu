@@ -14,6 +14,7 @@
 #include "../../include/fp.h"
 #include "fp_kernels.cuh"
 #include "fp_aligned.cuh"
+#include "fp_tma.cuh"
 
 using namespace fpk;
 
@@ -36,6 +37,9 @@ struct fp_ctx {
     int *ids_dev = nullptr;                    // [2 * ids_cap]: aligned ids, then direct ids
     int ids_cap = 0;
     bool aligned_attr_set = false;
+    // tensor maps of the TMA kernel: valid for one volume pointer
+    CUtensorMap tmap[2][kTmMaps];
+    const float *tmap_vol = nullptr;
     cudaStream_t last_stream = nullptr;
     bool counted = false;
     int last_launches = 0;
@@ -131,7 +135,7 @@ extern "C" fp_status fp_set_option(fp_ctx *c, int key, int value)
     if (!c) return FP_ERR_INVALID_ARG;
     switch (key) {
     case FP_OPT_KERNEL:
-        if (value < FP_KERNEL_AUTO || value > FP_KERNEL_ALIGNED) return fail(c, FP_ERR_INVALID_ARG, "bad kernel variant");
+        if (value < FP_KERNEL_AUTO || value > FP_KERNEL_TMA) return fail(c, FP_ERR_INVALID_ARG, "bad kernel variant");
         c->opt_kernel = value;
         return FP_OK;
     case FP_OPT_VOLATILE: c->opt_volatile = value != 0; return FP_OK;
@@ -228,8 +232,9 @@ static int plan_lane_v(const double *g, int nu, int nv, bool permuted)
 // 16-byte aligned volume (float4 loads along z).  The window bound is conservative: the largest
 // ray parameter |t| = |(i - s_m) / r_m| over all slices a batch can touch, times the r_z spread
 // of the rows of one block, plus the drift inside a batch, alignment and tap margins.
-static int plan_aligned(const fp_ctx *c, const float *vol, const double *g, int nu, int nv)
+static int plan_aligned(const fp_ctx *c, const float *vol, const double *g, int nu, int nv, int *tile_rows = nullptr)
 {
+    if (tile_rows) *tile_rows = 1 << 30;
     for (int k = 0; k < 12; ++k)
         if (!std::isfinite(g[k])) return 0;
     if (g[8] != 0.0 || g[9] != 0.0 || g[10] != 0.0 || g[11] == 0.0) return 0;
@@ -242,6 +247,8 @@ static int plan_aligned(const fp_ctx *c, const float *vol, const double *g, int 
     // per column: the slices whose slow-axis position can lie inside (-1, N_s) (one slice of slack on
     // either side), widened by one batch; the ray parameter t = (i - s_m) / r_m over them
     double rm_min = INFINITY, t_lo = INFINITY, t_hi = -INFINITY;
+    struct ColInfo { int m; double rt, dmax; };
+    std::vector<ColInfo> cols((size_t)nu, ColInfo{-1, 0.0, 0.0});
     for (int iu = 0; iu < nu; ++iu) {
         double r[2];
         for (int a = 0; a < 2; ++a) r[a] = ((g[3 + a] + iu * g[6 + a]) - c->G.origin[a]) / dl - s[a];
@@ -260,6 +267,7 @@ static int plan_aligned(const fp_ctx *c, const float *vol, const double *g, int 
         }
         if (i_a > i_b) continue;
         i_b += kAlSB;
+        cols[iu] = ColInfo{m, rt, std::max(std::fabs(i_a - s[m]), std::fabs(i_b - s[m]))};
         const double t_a = (i_a - s[m]) / rm, t_b = (i_b - s[m]) / rm;
         t_lo = std::min(t_lo, std::min(t_a, t_b));
         t_hi = std::max(t_hi, std::max(t_a, t_b));
@@ -275,6 +283,23 @@ static int plan_aligned(const fp_ctx *c, const float *vol, const double *g, int 
     const double dt_cols = t_max * (kAlTU * du / rm_min) + 4.0 / rm_min;
     const double span = t_max * (rows - 1) * std::fabs(g[11] / dl) + (kAlSB - 1) * (rz_max / rm_min) + dt_cols * rz_max;
     if (!(span < 1.0e6)) return 0;
+    if (tile_rows) {
+        // volume rows one block of fp_tma_kernel needs per slice: the columns of a block that share a driving
+        // axis spread over |i - s_m| (max r~_s - min r~_s) rows of the slice plane, plus the two taps
+        int rows = 0;
+        for (int iu0 = 0; iu0 < nu; iu0 += kTmTU)
+            for (int m = 0; m < 2; ++m) {
+                double lo = INFINITY, hi = -INFINITY, d = 0.0;
+                for (int iu = iu0; iu < std::min(nu, iu0 + kTmTU); ++iu)
+                    if (cols[iu].m == m) {
+                        lo = std::min(lo, cols[iu].rt);
+                        hi = std::max(hi, cols[iu].rt);
+                        d = std::max(d, cols[iu].dmax);
+                    }
+                if (lo <= hi) rows = std::max(rows, (int)std::min(d * (hi - lo), 1.0e6) + 3);
+            }
+        *tile_rows = rows;
+    }
     return (int)std::ceil(span) + 10;
 }
 
@@ -317,6 +342,56 @@ static fp_status launch_aligned(fp_ctx *c, const AlignedParams &A, int w, dim3 g
 }
 
 constexpr int kAlignedMaxW = 512;
+
+// Tensor maps of fp_tma_kernel over the caller's volume, dimensions (z, y, x): a box is kTmW voxels along z
+// and 8 or 12 rows along the slow transverse axis of the pass (y for m = x, x for m = y) of one slice.
+typedef CUresult (*tensor_map_encode_fn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
+                                         const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
+                                         CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+static fp_status build_tensor_maps(fp_ctx *c, const float *vol)
+{
+    if (c->tmap_vol == vol) return FP_OK;
+    static tensor_map_encode_fn encode = nullptr;
+    if (!encode) {
+        void *fn = nullptr;
+        cudaDriverEntryPointQueryResult q;
+        FP_CUDA(c, cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &q));
+        if (!fn || q != cudaDriverEntryPointSuccess) return fail(c, FP_ERR_UNSUPPORTED, "cuTensorMapEncodeTiled not available");
+        encode = (tensor_map_encode_fn)fn;
+    }
+    const cuuint64_t dims[3] = {(cuuint64_t)c->G.n[2], (cuuint64_t)c->G.n[1], (cuuint64_t)c->G.n[0]};
+    const cuuint64_t strides[2] = {(cuuint64_t)c->G.n[2] * 4, (cuuint64_t)c->G.n[2] * c->G.n[1] * 4};
+    const cuuint32_t estr[3] = {1, 1, 1};
+    for (int pass = 0; pass < 2; ++pass)
+        for (int big = 0; big < kTmMaps; ++big) {
+            const cuuint32_t rows = 4 + 2 * big;
+            const cuuint32_t box[3] = {(cuuint32_t)kTmW, pass == 0 ? rows : 1u, pass == 0 ? 1u : rows};
+            const CUresult r = encode(&c->tmap[pass][big], CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, (void *)vol, dims, strides, box,
+                                      estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                                      CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+            if (r != CUDA_SUCCESS) {
+                char buf[96];
+                snprintf(buf, sizeof buf, "cuTensorMapEncodeTiled failed (%d)", (int)r);
+                return fail(c, FP_ERR_CUDA, buf);
+            }
+        }
+    c->tmap_vol = vol;
+    return FP_OK;
+}
+
+template <int INTERP>
+static fp_status launch_tma(fp_ctx *c, const TmaParams &T, dim3 grid, cudaStream_t st)
+{
+    static bool attr_set = false;
+    if (!attr_set) {
+        FP_CUDA(c, cudaFuncSetAttribute(fp_tma_kernel<INTERP>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)tma_smem_bytes()));
+        attr_set = true;
+    }
+    fp_tma_kernel<INTERP><<<grid, kTmThreads, tma_smem_bytes(), st>>>(T);
+    FP_CUDA(c, cudaGetLastError());
+    return FP_OK;
+}
 
 static fp_status ensure_proj(fp_ctx *c, int n_proj)
 {
@@ -410,12 +485,14 @@ extern "C" fp_status fp_project(fp_ctx *c, const float *vol_dev, int n_proj, con
 
     // plan: which kernel takes which projection
     std::vector<int> ids_al, ids_di;
-    int w_al = 0;
+    int w_al = 0, rows_al = 0;
     for (int p = 0; p < n_proj; ++p) {
-        const int w = c->opt_kernel == FP_KERNEL_DIRECT ? 0 : plan_aligned(c, vol_dev, geom + 12 * (size_t)p, nu, nv);
+        int rows = 0;
+        const int w = c->opt_kernel == FP_KERNEL_DIRECT ? 0 : plan_aligned(c, vol_dev, geom + 12 * (size_t)p, nu, nv, &rows);
         if (w > 0 && w <= kAlignedMaxW) {
             ids_al.push_back(p);
             w_al = std::max(w_al, w);
+            rows_al = std::max(rows_al, rows);
         } else {
             ids_di.push_back(p);
         }
@@ -446,7 +523,25 @@ extern "C" fp_status fp_project(fp_ctx *c, const float *vol_dev, int n_proj, con
     FP_CUDA(c, cudaMemsetAsync(c->count_dev, 0, 2 * sizeof(unsigned long long), st));
     c->counted = c->opt_count != 0;
 
-    if (!ids_al.empty()) {
+    if (!ids_al.empty() && c->opt_kernel == FP_KERNEL_TMA && w_al <= kTmW && rows_al <= kTmNR) {
+        s = build_tensor_maps(c, vol_dev);
+        if (s != FP_OK) return s;
+        TmaParams T;
+        memcpy(T.map, c->tmap, sizeof T.map);
+        T.G = c->G;
+        T.proj = c->proj_dev;
+        T.ids = c->ids_dev;
+        T.out = out_dev;
+        T.sample_count = c->opt_count ? c->count_dev : nullptr;
+        T.err_flag = reinterpret_cast<unsigned int *>(c->count_dev + 1);
+        T.nu = nu;
+        T.nv = nv;
+        T.n_sel = (int)ids_al.size();
+        dim3 grid((unsigned)((nu + kTmTU - 1) / kTmTU), (unsigned)((nv + kTmRows - 1) / kTmRows), (unsigned)ids_al.size());
+        s = c->opt_interp == FP_INTERP_SPLINE ? launch_tma<1>(c, T, grid, st) : launch_tma<0>(c, T, grid, st);
+        if (s != FP_OK) return s;
+        c->last_launches += 1;
+    } else if (!ids_al.empty()) {
         AlignedParams A;
         A.G = c->G;
         A.vol = vol_dev;
@@ -513,7 +608,7 @@ extern "C" fp_status fp_last_sample_count(fp_ctx *c, unsigned long long *n)
     FP_CUDA(c, cudaStreamSynchronize(c->last_stream));
     unsigned long long h[2] = {0, 0};
     FP_CUDA(c, cudaMemcpy(h, c->count_dev, sizeof h, cudaMemcpyDeviceToHost));
-    if (h[1] != 0) return fail(c, FP_ERR_CUDA, "internal error: a staging window of fp_aligned_kernel did not fit (host plan too small)");
+    if (h[1] != 0) return fail(c, FP_ERR_CUDA, "internal error: a staging window or row tile of the aligned / TMA kernel did not fit (host plan too small)");
     *n = h[0];
     return FP_OK;
 }
@@ -522,9 +617,11 @@ extern "C" fp_status fp_plan(fp_ctx *c, const double *geom, int nu, int nv, int 
 {
     if (!c || !geom || !kernel || !window || !z_driven) return fail(c, FP_ERR_INVALID_ARG, "fp_plan: null argument");
     if (nu < 1 || nv < 1) return fail(c, FP_ERR_INVALID_ARG, "nu, nv must be >= 1");
-    const int w = c->opt_kernel == FP_KERNEL_DIRECT ? 0 : plan_aligned(c, nullptr, geom, nu, nv);
+    int rows = 0;
+    const int w = c->opt_kernel == FP_KERNEL_DIRECT ? 0 : plan_aligned(c, nullptr, geom, nu, nv, &rows);
     const bool al = w > 0 && w <= kAlignedMaxW;
     *kernel = al ? FP_KERNEL_ALIGNED : FP_KERNEL_DIRECT;
+    if (al && c->opt_kernel == FP_KERNEL_TMA && w <= kTmW && rows <= kTmNR) *kernel = FP_KERNEL_TMA;
     *window = al ? w : 0;
     *z_driven = has_z_driven(geom, nu, nv) ? 1 : 0;
     return FP_OK;

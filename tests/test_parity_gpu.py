@@ -361,3 +361,72 @@ def test_aligned_kernel_window_sizes_and_direct_kernel_agree(torch, fp):
         scale = np.abs(b).max()
         assert np.abs(a - b).max() <= 2e-5 * scale, (pitch, nv, np.abs(a - b).max(), scale)
     assert len(windows) >= 3                                # several of the 128 / 256 / 384 / 512 instantiations ran
+
+
+# ----------------------------------------------------------------------------- TMA-fed kernel (FP_KERNEL_TMA)
+
+def test_tma_kernel_parity(torch, fp, synth, oracle):
+    """fp_tma_kernel against the oracle: C1 in full, C2 on the poses whose row tile fits, the ragged /
+    mixed-axis / flipped / off-plane edge poses of the aligned kernel, spline weights."""
+    opt = [(fp.OPT_KERNEL, fp.KERNEL_TMA)]
+    cfg = synth.CONFIGS["C1"]
+    geom = synth.make_geometry(cfg)
+    with fp.Projector(*cfg.n, cfg.voxel_size, cfg.origin) as P:
+        P.set_option(fp.OPT_KERNEL, fp.KERNEL_TMA)
+        assert all(P.plan(g, cfg.nu, cfg.nv)[0] == fp.KERNEL_TMA for g in geom)
+    worst, _, _ = compare_full(torch, fp, oracle, synth.make_volume(cfg).numpy(), cfg.voxel_size, cfg.origin, geom,
+                               cfg.nu, cfg.nv, options=opt, what="C1 tma")
+    assert worst < 1.0
+    cfg = synth.CONFIGS["C2"]
+    geom = synth.make_geometry(cfg)
+    with fp.Projector(*cfg.n, cfg.voxel_size, cfg.origin) as P:
+        P.set_option(fp.OPT_KERNEL, fp.KERNEL_TMA)
+        sel = [p for p in range(cfg.n_proj) if P.plan(geom[p], cfg.nu, cfg.nv)[0] == fp.KERNEL_TMA]
+    assert len(sel) > 20
+    sel = sel[:: max(1, len(sel) // 8)]
+    worst, _, _ = compare_full(torch, fp, oracle, synth.make_volume(cfg).numpy(), cfg.voxel_size, cfg.origin, geom[sel],
+                               cfg.nu, cfg.nv, options=opt, what="C2 tma")
+    assert worst < 1.0
+    for nu, nv, interp in [(37, 300, 0), (66, 40, 1)]:
+        rng = np.random.default_rng(400 + nu)
+        shape = (21, 18, 24)
+        vol = rng.uniform(-1.0, 2.0, size=shape).astype(np.float32)
+        delta = 0.8
+        origin = tuple(-(n - 1) / 2.0 * delta + 0.17 * k for k, n in enumerate(shape))
+        pitch = 0.9 * 24 * delta * 2.2 / nv if nv > 100 else 0.55
+        geom = np.stack([aligned_pose(th, 40.0, 90.0, nu, nv, pitch, src_z=(k % 3 - 1) * 3.0,
+                                      det_shift=((k % 4) * 2.5, -(k % 2) * 3.0), flip_u=bool(k & 1), flip_v=bool(k & 2))
+                         for k, th in enumerate([0.0, math.pi / 4, 0.7853, 1.1, math.pi / 2, 2.5, math.pi, 3.9269908, 4.4, 5.9])])
+        with fp.Projector(*shape, delta, origin) as P:
+            P.set_option(fp.OPT_KERNEL, fp.KERNEL_TMA)
+            assert all(P.plan(g, nu, nv)[0] == fp.KERNEL_TMA for g in geom)
+        worst, _, _ = compare_full(torch, fp, oracle, vol, delta, origin, geom, nu, nv,
+                                   options=opt + [(fp.OPT_INTERP, interp)], kernel=interp, what="tma %dx%d" % (nu, nv))
+        assert worst < 1.0
+
+
+def test_tma_kernel_c3_sampled_and_fallback(torch, fp, synth, oracle):
+    cfg = synth.CONFIGS["C3"]
+    vol_t = synth.make_volume(cfg, device="cuda")
+    geom = synth.make_geometry(cfg)[[0, 44, 45, 46, 90, 135, 201, 359]]
+    with fp.Projector(*cfg.n, cfg.voxel_size, cfg.origin) as P:
+        P.set_option(fp.OPT_KERNEL, fp.KERNEL_TMA)
+        assert all(P.plan(g, cfg.nu, cfg.nv)[0] == fp.KERNEL_TMA for g in geom)
+        out = P.project(vol_t, geom, cfg.nu, cfg.nv)
+        torch.cuda.synchronize()
+        P.last_sample_count()                  # raises if a window or row tile overflowed
+        out = out.cpu().numpy()
+        # a pose that does not fit the tile (coarse detector columns) silently uses the aligned kernel
+        coarse = aligned_pose(0.8, cfg.sid, cfg.sdd, 96, 64, 3.0)
+        assert P.plan(coarse, 96, 64)[0] == fp.KERNEL_ALIGNED
+        P.project(vol_t, coarse[None], 96, 64)
+        torch.cuda.synchronize()
+        P.last_sample_count()
+    vol = vol_t.cpu().numpy()
+    rng = np.random.default_rng(99)
+    n = 30000
+    ids = np.stack([rng.integers(0, len(geom), n), rng.integers(0, cfg.nv, n), rng.integers(0, cfg.nu, n)], axis=1).astype(np.int32)
+    ov, om, pl, mg = oracle.project_rays(vol, cfg.voxel_size, cfg.origin, geom, ids, threads=oracle.host_cores())
+    g = out[ids[:, 0], ids[:, 1], ids[:, 2]]
+    tol = 2e-5 * np.abs(ov) + 1e-6 * pl * float(np.abs(vol).max())
+    assert np.all(np.abs(g - ov) <= tol), float(np.max(np.abs(g - ov) / np.maximum(tol, 1e-300)))
