@@ -62,15 +62,17 @@ typedef enum {
 
 /* fp_set_option keys.  Options are explicit; no environment variable changes behaviour. */
 enum {
-    /* Sampling-kernel variant.  FP_KERNEL_AUTO picks per projection: FP_KERNEL_ALIGNED (line
-     * staging in shared memory) for poses whose v vector is parallel to the volume's z axis and
-     * whose u vector is perpendicular to it and that have no z-driven ray (every circular orbit
-     * about z), FP_KERNEL_DIRECT (one thread per ray, four global taps per
-     * sample) for every other pose.  FP_KERNEL_DIRECT forces the direct kernel for all poses;
-     * FP_KERNEL_ALIGNED behaves like AUTO (poses it cannot take still use the direct kernel).
-     * FP_KERNEL_TMA: like AUTO, but calls whose aligned poses all fit a 256-voxel z window and 12 volume
-     * rows per block and slice are sampled by the TMA-fed kernel (tiles of the caller's volume copied to
-     * shared memory by cp.async.bulk.tensor, four taps per sample read from the tile). */
+    /* Sampling-kernel variant.  Poses whose v vector is parallel to the volume's z axis, whose u vector is
+     * perpendicular to it and that have no z-driven ray (every circular orbit about z)
+     * are "aligned"; all other poses always use FP_KERNEL_DIRECT (one thread per ray, four global taps per
+     * sample).  For the aligned poses of a call:
+     *   FP_KERNEL_AUTO     FP_KERNEL_TMA if they all fit a 256-voxel z window and 12 volume rows per block
+     *                      and slice, else FP_KERNEL_ALIGNED;
+     *   FP_KERNEL_TMA      the same as AUTO (tiles of the caller's volume copied to shared memory by
+     *                      cp.async.bulk.tensor, four taps per sample read from the tile);
+     *   FP_KERNEL_ALIGNED  always the line-staging kernel (two volume rows blended into shared memory per
+     *                      column and slice, two taps per sample);
+     *   FP_KERNEL_DIRECT   the direct kernel for every pose. */
     FP_OPT_KERNEL = 1,
     /* 1 (default): the volume contents may have changed since the last call, internal copies
      * are rebuilt by every fp_project that needs them.  0: internal copies made by fp_prepare

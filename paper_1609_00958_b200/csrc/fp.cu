@@ -523,7 +523,7 @@ extern "C" fp_status fp_project(fp_ctx *c, const float *vol_dev, int n_proj, con
     FP_CUDA(c, cudaMemsetAsync(c->count_dev, 0, 2 * sizeof(unsigned long long), st));
     c->counted = c->opt_count != 0;
 
-    if (!ids_al.empty() && c->opt_kernel == FP_KERNEL_TMA && w_al <= kTmW && rows_al <= kTmNR) {
+    if (!ids_al.empty() && c->opt_kernel != FP_KERNEL_ALIGNED && w_al <= kTmW && rows_al <= kTmNR) {
         s = build_tensor_maps(c, vol_dev);
         if (s != FP_OK) return s;
         TmaParams T;
@@ -621,7 +621,7 @@ extern "C" fp_status fp_plan(fp_ctx *c, const double *geom, int nu, int nv, int 
     const int w = c->opt_kernel == FP_KERNEL_DIRECT ? 0 : plan_aligned(c, nullptr, geom, nu, nv, &rows);
     const bool al = w > 0 && w <= kAlignedMaxW;
     *kernel = al ? FP_KERNEL_ALIGNED : FP_KERNEL_DIRECT;
-    if (al && c->opt_kernel == FP_KERNEL_TMA && w <= kTmW && rows <= kTmNR) *kernel = FP_KERNEL_TMA;
+    if (al && c->opt_kernel != FP_KERNEL_ALIGNED && w <= kTmW && rows <= kTmNR) *kernel = FP_KERNEL_TMA;
     *window = al ? w : 0;
     *z_driven = has_z_driven(geom, nu, nv) ? 1 : 0;
     return FP_OK;

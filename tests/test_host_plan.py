@@ -25,7 +25,9 @@ def test_circular_orbits_take_the_aligned_kernel(name, wmax):
         ws = []
         for p in range(0, cfg.n_proj, max(1, cfg.n_proj // 45)):
             k, w, z = P.plan(geom[p], cfg.nu, cfg.nv)
-            assert k == fp.KERNEL_ALIGNED and not z, (name, p)
+            assert k in (fp.KERNEL_ALIGNED, fp.KERNEL_TMA) and not z, (name, p)
+            # the TMA-fed kernel only where its 256-voxel window holds the block's rows
+            assert (k == fp.KERNEL_TMA) <= (w <= 256), (name, p, w)
             ws.append(w)
         # the window must hold the z extent of one block's rows (at most 256 of them)
         assert 16 <= max(ws) <= wmax, (name, max(ws))
@@ -48,7 +50,10 @@ def test_aligned_kernel_is_refused_when_its_preconditions_fail():
     cfg = synth.CONFIGS["C2"]
     g = circular_pose(0.3, cfg.sid, cfg.sdd, cfg.nu, cfg.nv, cfg.pitch)
     with fp.Projector(*cfg.n, cfg.voxel_size, cfg.origin) as P:
+        assert P.plan(g, cfg.nu, cfg.nv)[0] in (fp.KERNEL_ALIGNED, fp.KERNEL_TMA)
+        P.set_option(fp.OPT_KERNEL, fp.KERNEL_ALIGNED)
         assert P.plan(g, cfg.nu, cfg.nv)[0] == fp.KERNEL_ALIGNED
+        P.set_option(fp.OPT_KERNEL, fp.KERNEL_AUTO)
         # a rolled detector: u picks up a z component
         r = g.copy()
         r[6:9] = 0.999 * g[6:9] + 0.04 * g[9:12]

@@ -332,9 +332,11 @@ def test_aligned_kernel_edge_cases(torch, fp, oracle, nu, nv, interp):
                                   det_shift=((k % 4) * 2.5, -(k % 2) * 3.0), flip_u=bool(k & 1), flip_v=bool(k & 2)))
     geom = np.stack(poses)
     with fp.Projector(*shape, delta, origin) as P:
+        P.set_option(fp.OPT_KERNEL, fp.KERNEL_ALIGNED)
         assert all(P.plan(g, nu, nv)[0] == fp.KERNEL_ALIGNED for g in geom)
     worst, out, om = compare_full(torch, fp, oracle, vol, delta, origin, geom, nu, nv,
-                                  options=[(fp.OPT_INTERP, interp)], kernel=interp, what="aligned %dx%d" % (nu, nv))
+                                  options=[(fp.OPT_KERNEL, fp.KERNEL_ALIGNED), (fp.OPT_INTERP, interp)], kernel=interp,
+                                  what="aligned %dx%d" % (nu, nv))
     assert worst < 1.0
     assert set(np.unique(om[:, 0])) <= {0, 1}
     if nv > 100:
@@ -352,6 +354,7 @@ def test_aligned_kernel_window_sizes_and_direct_kernel_agree(torch, fp):
     for pitch, nv in [(0.7, 64), (1.5, 192), (2.0, 256), (2.5, 270)]:
         geom = np.stack([aligned_pose(th, cfg.sid, cfg.sdd, 96, nv, pitch) for th in (0.2, 0.8, 2.0, 4.0)])
         with fp.Projector(*cfg.n, cfg.voxel_size, cfg.origin) as P:
+            P.set_option(fp.OPT_KERNEL, fp.KERNEL_ALIGNED)
             plans = [P.plan(g, 96, nv) for g in geom]
             assert all(k == fp.KERNEL_ALIGNED for k, _, _ in plans), plans
             windows.add((max(w for _, w, _ in plans) + 127) // 128)
