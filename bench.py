@@ -31,6 +31,9 @@ METRIC = "512^3 cone-beam projections/s"
 UNIT = "projections/s"
 TAP_BYTES = 16           # 4 taps x 4 B per sample: the paper's "memory access rate"
 FALLBACK_HBM_GBS = 6650.0
+# dram__bytes_read.sum + dram__bytes_write.sum of one launch, from the committed ncu --set full captures
+# (profiles/r1_02_aligned_kernel_c3.md, profiles/r1_03_tma_kernel_c3.md); None where no capture exists
+NCU_TRAFFIC_BYTES = {("C3", "fp_aligned_kernel"): 201.51e9, ("C3", "fp_tma_kernel"): 273.31e9}
 
 
 def measured_peaks():
@@ -291,6 +294,9 @@ def main():
             dist.destroy_process_group()
         return 0
 
+    # which sampling kernel the library's plan picks for this workload (fp_plan, host only)
+    kernel_name = {fp.KERNEL_DIRECT: "fp_direct_kernel", fp.KERNEL_ALIGNED: "fp_aligned_kernel",
+                   fp.KERNEL_TMA: "fp_tma_kernel"}[P.plan(geom[0], cfg.nu, cfg.nv)[0]]
     peaks, peak_kind = measured_peaks()
     vol_bytes = vol.numel() * 4
     out_bytes_per_proj = cfg.nu * cfg.nv * 4
@@ -299,8 +305,8 @@ def main():
     kernel_ms = ms_per_step            # one sampling launch per fp_project; the step is that launch
     achieved = algo_bytes_per_step / (kernel_ms * 1e-3) / 1e9
     roofline = {"bound": "hbm", "achieved": achieved, "peak": peaks["hbm_gbs"], "unit": "GB/s",
-                "frac": achieved / peaks["hbm_gbs"], "traffic": None, "peak_kind": peak_kind,
-                "kernel": "fp_aligned_kernel" if (cfg.orbit == "circular" and args.kernel != 1) else "fp_direct_kernel", "algorithmic_bytes_per_launch": algo_bytes_per_step // max(1, (cfg.n_proj + batch - 1) // batch)}
+                "frac": achieved / peaks["hbm_gbs"], "traffic": NCU_TRAFFIC_BYTES.get((cfg.name, kernel_name)), "peak_kind": peak_kind,
+                "kernel": kernel_name, "algorithmic_bytes_per_launch": algo_bytes_per_step // max(1, (cfg.n_proj + batch - 1) // batch)}
 
     cpu_baseline = None
     parity = None
