@@ -99,7 +99,7 @@ class ClockSampler:
         return out
 
 
-def oracle_sample(cfg, geom, vol_np, max_seconds=20.0):
+def oracle_sample(cfg, geom, vol_np, max_seconds=20.0, kernel=0):
     """Time the oracle, as it stands, on a bounded sample of the workload: whole detector rows of
     projection 0 and of the projection at 1/8 of the orbit (both driving axes for circular
     orbits), using every host core.  Returns (projections/s, samples/s, cores, description,
@@ -116,12 +116,12 @@ def oracle_sample(cfg, geom, vol_np, max_seconds=20.0):
         return np.stack([p.ravel(), v.ravel(), u.ravel()], axis=1).astype(np.int32)
     ids = ids_for(rows_cal)
     t0 = time.perf_counter()
-    oracle.project_rays(vol_np, cfg.voxel_size, cfg.origin, geom, ids, threads=cores)
+    oracle.project_rays(vol_np, cfg.voxel_size, cfg.origin, geom, ids, kernel=kernel, threads=cores)
     t_cal = time.perf_counter() - t0
     rows = int(max(rows_cal, min(cfg.nv, rows_cal * max_seconds / max(t_cal, 1e-3))))
     ids = ids_for(rows)
     t0 = time.perf_counter()
-    val, mfl, pl, mg = oracle.project_rays(vol_np, cfg.voxel_size, cfg.origin, geom, ids, threads=cores)
+    val, mfl, pl, mg = oracle.project_rays(vol_np, cfg.voxel_size, cfg.origin, geom, ids, kernel=kernel, threads=cores)
     dt = time.perf_counter() - t0
     n_samples = int(np.maximum(mfl[:, 2] - mfl[:, 1] + 1, 0).sum())
     rays_per_proj = cfg.nu * cfg.nv
@@ -144,7 +144,7 @@ def run_reference(args):
     vals = []
     desc, cores = "", 0
     for k in range(args.warmup + args.steps):
-        pps, sps, cores, desc, *_ = oracle_sample(cfg, geom, vol, max_seconds=min(20.0, budget))
+        pps, sps, cores, desc, *_ = oracle_sample(cfg, geom, vol, max_seconds=min(20.0, budget), kernel=1 if args.interp == "spline" else 0)
         if k >= args.warmup:
             vals.append((pps, sps))
     pps = statistics.median(v[0] for v in vals)
@@ -193,6 +193,8 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--kernel", type=int, default=0, help="FP_OPT_KERNEL value (0 = auto)")
+    ap.add_argument("--interp", default="linear", choices=["linear", "spline"],
+                    help="interpolation kernel: GJP_lin (PAPER.md:150 Eq. 13, the headline) or GJP_spl (:152 Eq. 14)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 0)
     if args.impl == "reference":
@@ -221,6 +223,8 @@ def main():
     P = fp.Projector(*cfg.n, cfg.voxel_size, cfg.origin)
     if args.kernel:
         P.set_option(fp.OPT_KERNEL, args.kernel)
+    interp = fp.INTERP_SPLINE if args.interp == "spline" else fp.INTERP_LINEAR
+    P.set_option(fp.OPT_INTERP, interp)
     stream = torch.cuda.current_stream()
 
     def step():
@@ -273,6 +277,9 @@ def main():
         vol_h = vol.cpu().pin_memory()
         out_h = torch.empty((cfg.n_proj, cfg.nv, cfg.nu), dtype=torch.float32).pin_memory()
         P2 = fp.Projector(*cfg.n, cfg.voxel_size, cfg.origin)
+        P2.set_option(fp.OPT_INTERP, interp)
+        if args.kernel:
+            P2.set_option(fp.OPT_KERNEL, args.kernel)
         P2.project_host(vol_h, geom, cfg.nu, cfg.nv, out_host=out_h)          # warm-up (allocations)
         n_e2e = max(1, min(args.steps, 3))
         barrier()
@@ -312,7 +319,7 @@ def main():
     parity = None
     if not args.no_cpu_baseline and world == 1:
         vol_np = vol.cpu().numpy()
-        pps, sps, cores, desc, ids, val, mfl, pl, mg = oracle_sample(cfg, geom, vol_np, max_seconds=15.0)
+        pps, sps, cores, desc, ids, val, mfl, pl, mg = oracle_sample(cfg, geom, vol_np, max_seconds=15.0, kernel=1 if args.interp == "spline" else 0)
         cpu_baseline = {"value": pps, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc,
                         "gsamples_per_s": sps / 1e9, "extrapolated_from_sample": True}
         g = out[torch.from_numpy(ids[:, 0].astype(np.int64)).cuda(), torch.from_numpy(ids[:, 1].astype(np.int64)).cuda(),
@@ -327,7 +334,7 @@ def main():
         "config": {"workload": workload_name(cfg), "projections_per_call": batch, "replicas": world,
                    "l2_policy": "inputs larger than L2 (volume %d MB, output %d MB per step; L2 126 MB)" % (
                        vol_bytes >> 20, (cfg.n_proj * out_bytes_per_proj) >> 20),
-                   "layout_stage_in_timed_region": True},
+                   "layout_stage_in_timed_region": True, "interpolation": args.interp},
         "gsamples_per_s": samples_per_s / 1e9,
         "samples_per_step": samples,
         "tap_access_rate_gbs": TAP_BYTES * samples_per_s / 1e9,
