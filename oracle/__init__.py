@@ -60,6 +60,9 @@ def lib():
                                        ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_int,
                                        dp, ip, dp, dp]
         L.jo_project_block.restype = None
+        L.jo_backproject.argtypes = [dp, cip, ctypes.c_double, dp, dp, ctypes.c_int, ctypes.c_int, ctypes.c_int,
+                                     ctypes.c_int, dp]
+        L.jo_backproject.restype = None
         _lib = L
     return _lib
 
@@ -180,6 +183,34 @@ def project(vol, voxel_size, origin, geom, nu, nv, kernel: int = KERNEL_LIN, thr
         with ThreadPoolExecutor(max_workers=threads) as ex:
             list(ex.map(run, jobs))
     return values, mfl, pathlen
+
+
+def backproject(proj, shape, voxel_size, origin, geom, kernel: int = KERNEL_LIN, threads: int = 1):
+    """Exact transpose of ``project`` (jo_backproject): proj f64[n_proj][nv][nu] -> volume f64[nx][ny][nz].
+    ``threads`` > 1 splits the projections over a thread pool, each thread into its own accumulator."""
+    y = np.ascontiguousarray(proj, dtype=np.float64)
+    assert y.ndim == 3
+    n_proj, nv, nu = y.shape
+    geom = np.ascontiguousarray(geom, dtype=np.float64).reshape(-1, 12)
+    assert geom.shape[0] == n_proj
+    origin = np.ascontiguousarray(origin, dtype=np.float64)
+    n = (ctypes.c_int * 3)(*[int(k) for k in shape])
+    lib()
+
+    def run(lo, hi):
+        out = np.zeros(tuple(int(k) for k in shape), dtype=np.float64)
+        if hi > lo:
+            lib().jo_backproject(_dptr(y[lo:hi]), n, float(voxel_size), _dptr(origin), _dptr(geom[lo:hi]), kernel,
+                                 hi - lo, nu, nv, _dptr(out))
+        return out
+
+    threads = max(1, min(threads, n_proj))
+    if threads == 1:
+        return run(0, n_proj)
+    cuts = np.linspace(0, n_proj, threads + 1).astype(int)
+    with ThreadPoolExecutor(max_workers=threads) as ex:
+        parts = list(ex.map(lambda k: run(int(cuts[k]), int(cuts[k + 1])), range(threads)))
+    return sum(parts[1:], parts[0])
 
 
 def host_cores() -> int:

@@ -14,7 +14,8 @@
  *
  * Parity status: every function here is pinned by tests/test_oracle_pins.py
  * (closed forms, invariants, a library trilinear routine, brute force on tiny
- * inputs, a hand-worked example) -- nothing is "parity unpinned".
+ * inputs, a hand-worked example; the back-projection voxel by voxel against the pinned
+ * forward projection of unit volumes) -- nothing is "parity unpinned".
  *
  * What is computed (PAPER.md line numbers; section / equation in brackets):
  *   r = d - s                                   :77  [sec 2.1, Eq. 1]
@@ -261,4 +262,61 @@ void jo_project_block(const float *vol, const int n[3], double delta, const doub
             if (pathlen) pathlen[q] = delta * L * (double)(t[2] - t[1] + 1);
             if (margins) { margins[2 * q] = mg[0]; margins[2 * q + 1] = mg[1]; }
         }
+}
+
+/*
+ * jo_backproject: the exact transpose of jo_project_block over whole projections
+ * (SURVEY.md 8(f) #2; PAPER.md:27, :308, :367 -- iterative methods pair the projector with
+ * its back-projection).  With A the linear map volume -> projections defined by
+ * jo_ray_grid (same set-up, same in-volume predicate, same taps and weights, times the voxel
+ * pitch), this accumulates  vol_out += A^T proj :  every tap (voxel) of every sample of every
+ * ray receives  delta * ||r~|| * w * w * proj[ray].  Taps outside 0..N-1 belong to the zero
+ * extension (reading #2) and receive nothing.
+ *   proj     [n_proj][nv][nu]  fp64, u fastest
+ *   vol_out  [nx][ny][nz]      fp64, z fastest; NOT cleared here
+ */
+void jo_backproject(const double *proj, const int n[3], double delta, const double origin[3],
+                    const double *geom, int kernel, int n_proj, int nu, int nv, double *vol_out)
+{
+    int p, iu, iv;
+    for (p = 0; p < n_proj; ++p)
+        for (iv = 0; iv < nv; ++iv)
+            for (iu = 0; iu < nu; ++iu) {
+                double s[3], d[3], rt[3], L = 0.0;
+                int m = 0, t1, t2, i;
+                const double y = proj[((size_t)p * (size_t)nv + (size_t)iv) * (size_t)nu + (size_t)iu];
+                jo_pixel_to_grid(geom + 12 * (size_t)p, delta, origin, iu, iv, s, d);
+                if (!jo_setup(s, d, &m, rt, &L))
+                    continue;
+                t1 = (m + 1) % 3;
+                t2 = (m + 2) % 3;
+                for (i = 0; i < n[m]; ++i) {
+                    double pc[3], w0[3], w1[3];
+                    long fl[3];
+                    int a, b;
+                    pc[m] = (double)i;
+                    pc[t1] = jo_pt(s, rt, m, t1, i);
+                    pc[t2] = jo_pt(s, rt, m, t2, i);
+                    /* the predicate of step 6; a sample outside it has no tap inside the volume anyway */
+                    if (!((-1.0 < pc[t1]) && (pc[t1] < (double)n[t1]) && (-1.0 < pc[t2]) && (pc[t2] < (double)n[t2])))
+                        continue;
+                    for (a = 0; a < 3; ++a) {
+                        double f = floor(pc[a]);
+                        fl[a] = (long)f;
+                        w0[a] = jo_w(kernel, pc[a] - f);
+                        w1[a] = 1.0 - w0[a];
+                    }
+                    for (a = 0; a < 2; ++a)
+                        for (b = 0; b < 2; ++b) {
+                            long idx[3];
+                            idx[m] = fl[m];
+                            idx[t1] = fl[t1] + a;
+                            idx[t2] = fl[t2] + b;
+                            if (idx[0] < 0 || idx[1] < 0 || idx[2] < 0 || idx[0] >= n[0] || idx[1] >= n[1] || idx[2] >= n[2])
+                                continue;
+                            vol_out[((size_t)idx[0] * (size_t)n[1] + (size_t)idx[1]) * (size_t)n[2] + (size_t)idx[2]] +=
+                                delta * L * (a ? w1[t1] : w0[t1]) * (b ? w1[t2] : w0[t2]) * y;
+                        }
+                }
+            }
 }

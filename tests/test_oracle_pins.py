@@ -481,3 +481,68 @@ def test_golden_regression(oracle):
         fa, fb = a.split(), b.split()
         assert fa[:6] == fb[:6]
         assert abs(float(fa[6]) - float(fb[6])) <= 1e-12 * max(1.0, abs(float(fa[6])))
+
+
+# ----------------------------------------------------------------------------- back-projection oracle
+
+def _bp_poses(shape, delta, nu, nv):
+    """Three poses whose rays are x-, y- and z-driven, detector slightly larger than the volume's shadow."""
+    ctr = np.zeros(3)
+    poses = []
+    for src, u, v in [((-40.0, 3.0, 2.0), (0.0, 1.0, 0.1), (0.0, -0.1, 1.0)),
+                      ((2.0, 38.0, -3.0), (1.0, 0.0, 0.2), (-0.2, 0.0, 1.0)),
+                      ((3.0, -2.0, 41.0), (1.0, 0.15, 0.0), (-0.15, 1.0, 0.0))]:
+        S = np.array(src)
+        n = (ctr - S) / np.linalg.norm(ctr - S)
+        C = S + 70.0 * n
+        U = 0.9 * np.array(u) / np.linalg.norm(u)
+        V = 0.9 * np.array(v) / np.linalg.norm(v)
+        poses.append(np.concatenate([S, C - (nu - 1) / 2 * U - (nv - 1) / 2 * V, U, V]))
+    return np.stack(poses)
+
+
+@pytest.mark.parametrize("kernel", [0, 1])
+def test_backprojection_is_the_transpose_voxel_by_voxel(oracle, kernel):
+    """(A^T y)[v] = <A e_v, y> for EVERY voxel v of a tiny grid: the back-projection oracle against the
+    pinned forward oracle applied to unit volumes (the definition of the transpose, nothing shared but
+    the ray set-up)."""
+    rng = np.random.default_rng(71)
+    shape, delta, nu, nv = (4, 5, 3), 0.8, 9, 8
+    origin = tuple(-(n - 1) / 2.0 * delta + 0.1 * k for k, n in enumerate(shape))
+    geom = _bp_poses(shape, delta, nu, nv)
+    y = rng.uniform(-1.0, 2.0, size=(len(geom), nv, nu))
+    bp = oracle.backproject(y, shape, delta, origin, geom, kernel=kernel)
+    assert bp.shape == shape
+    seen_axes = set()
+    for v in itertools.product(*[range(n) for n in shape]):
+        e = np.zeros(shape, dtype=np.float32)
+        e[v] = 1.0
+        fwd, mfl, _ = oracle.project(e, delta, origin, geom, nu, nv, kernel=kernel)
+        seen_axes |= set(np.unique(mfl[..., 0]))
+        assert abs(bp[v] - float((fwd * y).sum())) <= 1e-12 * max(1.0, abs(bp[v])), v
+    assert seen_axes == {0, 1, 2}
+    assert np.abs(bp).max() > 0.1
+
+
+def test_backprojection_adjoint_identity_and_linearity(oracle):
+    rng = np.random.default_rng(72)
+    shape, delta, nu, nv = (11, 9, 12), 0.7, 21, 17
+    origin = tuple(-(n - 1) / 2.0 * delta for n in shape)
+    geom = _bp_poses(shape, delta, nu, nv)
+    x = rng.uniform(-1.0, 1.0, size=shape).astype(np.float32)
+    y1 = rng.uniform(-1.0, 1.0, size=(len(geom), nv, nu))
+    y2 = rng.uniform(-1.0, 1.0, size=(len(geom), nv, nu))
+    ax, _, _ = oracle.project(x, delta, origin, geom, nu, nv)
+    b1 = oracle.backproject(y1, shape, delta, origin, geom)
+    b2 = oracle.backproject(y2, shape, delta, origin, geom, threads=3)
+    lhs, rhs = float((ax * y1).sum()), float((x.astype(np.float64) * b1).sum())
+    assert abs(lhs - rhs) <= 1e-11 * max(abs(lhs), 1.0)
+    b12 = oracle.backproject(2.0 * y1 - 3.0 * y2, shape, delta, origin, geom)
+    assert np.allclose(b12, 2.0 * b1 - 3.0 * b2, rtol=0, atol=1e-11)
+    # weights are non-negative: a non-negative projection back-projects to a non-negative volume,
+    # and <A 1, y> = sum(A^T y)
+    ones = np.ones(shape, dtype=np.float32)
+    a1, _, _ = oracle.project(ones, delta, origin, geom, nu, nv)
+    bp = oracle.backproject(np.abs(y1), shape, delta, origin, geom)
+    assert bp.min() >= 0.0
+    assert abs(float((a1 * np.abs(y1)).sum()) - float(bp.sum())) <= 1e-10 * float(bp.sum())
