@@ -135,6 +135,19 @@ fp_status fp_project_host(fp_ctx *ctx, const float *vol_host, int n_proj, const 
                           int nu, int nv, float *out_host);
 
 /*
+ * fp_backproject: the exact transpose of fp_project (SURVEY.md section 8(f) #2; PAPER.md:27, :308, :367:
+ * iterative reconstruction pairs the projector with its back-projection).  With A the linear map
+ * volume -> projections that fp_project computes for these poses, writes vol_out = A^T proj: every tap of
+ * every sample of every ray receives voxel_size * ||r~|| * w * w * proj[ray] (same set-up, slices, taps and
+ * weights; FP_OPT_INTERP applies).  fp32 reductions in arbitrary order: results are reproducible only to
+ * fp32 rounding of the sum.
+ *   proj_dev     device, fp32 [n_proj][nv][nu]
+ *   vol_out_dev  device, fp32 [nx][ny][nz], fully overwritten (cleared first, also for n_proj = 0)
+ */
+fp_status fp_backproject(fp_ctx *ctx, const float *proj_dev, int n_proj, const double *geom_host,
+                         int nu, int nv, float *vol_out_dev, fp_stream stream);
+
+/*
  * fp_ray_ranges: per-ray set-up only (PAPER.md:71-106 Eqs. 1-6, Alg. 1 l.1-5, :213): writes
  * { m, i_first, i_last } per pixel; a miss is { m, 0, -1 }, the degenerate ray { 0, 0, -1 }.
  * The decisions are taken in IEEE fp64 in the operation order DESIGN.md fixes, so they are

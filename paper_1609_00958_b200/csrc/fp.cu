@@ -585,6 +585,40 @@ extern "C" fp_status fp_project(fp_ctx *c, const float *vol_dev, int n_proj, con
     return FP_OK;
 }
 
+extern "C" fp_status fp_backproject(fp_ctx *c, const float *proj_dev, int n_proj, const double *geom, int nu, int nv,
+                                    float *vol_out_dev, fp_stream stream)
+{
+    fp_status s = check_project_args(c, proj_dev, n_proj, geom, nu, nv, vol_out_dev);
+    if (s != FP_OK) return s;
+    if (!vol_out_dev) return fail(c, FP_ERR_INVALID_ARG, "null pointer");
+    cudaStream_t st = (cudaStream_t)stream;
+    c->last_launches = 0;
+    c->last_stream = st;
+    c->counted = false;
+    FP_CUDA(c, cudaMemsetAsync(vol_out_dev, 0, n_voxels(c) * sizeof(float), st));
+    if (n_proj == 0) return FP_OK;
+    s = upload_geometry(c, n_proj, geom, nu, nv, false, st);
+    if (s != FP_OK) return s;
+    BackprojectParams B;
+    B.G = c->G;
+    fill_layouts(c, vol_out_dev, false, B.lay);
+    B.proj = c->proj_dev;
+    B.in = proj_dev;
+    B.nu = nu;
+    B.nv = nv;
+    B.n_proj = n_proj;
+    const unsigned gl = (unsigned)((std::max(nu, nv) + kTileLane - 1) / kTileLane);
+    const unsigned gr = (unsigned)((std::max(nu, nv) + kTileRow - 1) / kTileRow);
+    dim3 grid(gl, gr, (unsigned)n_proj);
+    if (c->opt_interp == FP_INTERP_SPLINE)
+        fp_backproject_kernel<1><<<grid, kDirectThreads, 0, st>>>(B);
+    else
+        fp_backproject_kernel<0><<<grid, kDirectThreads, 0, st>>>(B);
+    FP_CUDA(c, cudaGetLastError());
+    c->last_launches += 1;
+    return FP_OK;
+}
+
 extern "C" fp_status fp_ray_ranges(fp_ctx *c, int n_proj, const double *geom, int nu, int nv, int32_t *mfl_dev,
                                    fp_stream stream)
 {

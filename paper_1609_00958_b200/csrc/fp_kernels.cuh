@@ -189,6 +189,75 @@ fp_direct_kernel(const __grid_constant__ ProjectParams P)
     if (P.sample_count) block_count_samples(P.sample_count, n_samples);
 }
 
+// ------------------------------------------------------------------------------------------
+// Back-projection (the exact transpose of the sampling loop, PAPER.md:27,
+// :308, :367): one thread per ray, same set-up, same slices, same four taps and product weights
+// as fp_direct_kernel; instead of gathering vol[tap] * w it scatters delta ||r~|| w proj[ray]
+// into vol_out[tap] with fp32 reductions in L2 (RED.ADD.F32).  Taps outside the volume belong to
+// the zero extension (reading #2) and receive nothing.
+// ------------------------------------------------------------------------------------------
+struct BackprojectParams {
+    GridDesc G;
+    AxisLayout lay[3];                 // the OUTPUT volume [nx][ny][nz], indexed by the driving axis m
+    const ProjDesc *proj;
+    const float *in;                   // [n_proj][nv][nu]
+    int nu, nv, n_proj;
+};
+
+template <int INTERP>
+__global__ void __launch_bounds__(kDirectThreads)
+fp_backproject_kernel(const __grid_constant__ BackprojectParams P)
+{
+    const int proj = blockIdx.z;
+    const ProjDesc *pd = P.proj + proj;
+    const int lane = threadIdx.x & 31, row = threadIdx.x >> 5;
+    const bool lane_v = pd->lane_v != 0;
+    const int a_lane = blockIdx.x * kTileLane + lane;
+    const int a_row = blockIdx.y * kTileRow + row;
+    const int iu = lane_v ? a_row : a_lane;
+    const int iv = lane_v ? a_lane : a_row;
+    if (iu >= P.nu || iv >= P.nv) return;
+    const RaySetup R = ray_setup(pd->g, P.G, iu, iv);
+    if (R.i_last < R.i_first) return;
+    const float y = P.in[((size_t)proj * P.nv + iv) * P.nu + iu] * (float)(P.G.delta * R.L);
+    if (y == 0.0f) return;
+    const AxisLayout &A = P.lay[R.m];
+    float *__restrict__ base = const_cast<float *>(A.base);
+    const long long si = A.si, ss = A.ss, sf = A.sf;
+    const unsigned n_s = (unsigned)A.n_s, n_f = (unsigned)A.n_f;
+    const float2 r2 = make_float2((float)R.rt_a, (float)R.rt_b);
+    const float2 kMagic2 = make_float2(12582912.0f, 12582912.0f), kNegMagic2 = make_float2(-12582912.0f, -12582912.0f);
+    const float2 kNegOne2 = make_float2(-1.0f, -1.0f), kOne2 = make_float2(1.0f, 1.0f);
+    for (int s0 = R.i_first; s0 <= R.i_last; s0 += kSegment) {
+        const int s1 = min(s0 + kSegment - 1, R.i_last);
+        const int ic = (s0 + s1) >> 1;
+        const double pa = p_of_i(R.s_a, R.s_m, R.rt_a, ic), pb = p_of_i(R.s_b, R.s_m, R.rt_b, ic);
+        const double fa = floor(pa), fb = floor(pb);
+        const int ja = (int)fa, kb = (int)fb;
+        const float2 a2 = make_float2((float)(pa - fa), (float)(pb - fb));
+        float *qseg = base + (long long)ja * ss + (long long)kb * sf + (long long)s0 * si;
+        float2 fi = make_float2((float)(s0 - ic), (float)(s0 - ic));
+        for (int i = s0; i <= s1; ++i) {
+            const float2 p = __ffma2_rn(fi, r2, a2);
+            fi = __fadd2_rn(fi, kOne2);
+            const float2 x = __fadd2_rd(p, kMagic2);
+            const float2 d = __ffma2_rn(__fadd2_rn(x, kNegMagic2), kNegOne2, p);
+            const int jl = __float_as_int(x.x) - 0x4B400000, kl = __float_as_int(x.y) - 0x4B400000;
+            const float u1 = ceil_weight<INTERP>(d.x), u2 = ceil_weight<INTERP>(d.y);
+            float *q = qseg + (long long)jl * ss + (long long)kl * sf;
+            qseg += si;
+            const int j = ja + jl, k = kb + kl;
+            const bool j0 = (unsigned)j < n_s, j1 = (unsigned)(j + 1) < n_s;
+            const bool k0 = (unsigned)k < n_f, k1 = (unsigned)(k + 1) < n_f;
+            const float ya = y * (1.0f - u1), yb = y * u1;      // rows j, j + 1
+            if (j0 && k0) atomicAdd(q, ya * (1.0f - u2));
+            if (j0 && k1) atomicAdd(q + sf, ya * u2);
+            if (j1 && k0) atomicAdd(q + ss, yb * (1.0f - u2));
+            if (j1 && k1) atomicAdd(q + ss + sf, yb * u2);
+        }
+    }
+}
+
 // Ray-range export (parity / debug): { m, i_first, i_last } per pixel.
 __global__ void __launch_bounds__(256)
 fp_ranges_kernel(GridDesc G, const ProjDesc *__restrict__ proj, int nu, int nv, int32_t *__restrict__ mfl)

@@ -24,7 +24,7 @@ INTERP_LINEAR, INTERP_SPLINE = 0, 1
 
 # every symbol include/fp.h declares (tests check the library exports all of them)
 SYMBOLS = ["fp_create", "fp_destroy", "fp_set_option", "fp_get_option", "fp_prepare", "fp_project",
-           "fp_project_host", "fp_ray_ranges", "fp_plan", "fp_last_sample_count", "fp_last_launch_count",
+           "fp_project_host", "fp_backproject", "fp_ray_ranges", "fp_plan", "fp_last_sample_count", "fp_last_launch_count",
            "fp_status_string", "fp_last_error", "fp_version"]
 
 
@@ -60,12 +60,13 @@ def load(build_if_missing: bool = True):
     L.fp_prepare.argtypes = [vp, vp, vp]
     L.fp_project.argtypes = [vp, vp, i, dp, i, i, vp, vp]
     L.fp_project_host.argtypes = [vp, vp, i, dp, i, i, vp]
+    L.fp_backproject.argtypes = [vp, vp, i, dp, i, i, vp, vp]
     L.fp_ray_ranges.argtypes = [vp, i, dp, i, i, vp, vp]
     L.fp_plan.argtypes = [vp, dp, i, i, ctypes.POINTER(i), ctypes.POINTER(i), ctypes.POINTER(i)]
     L.fp_last_sample_count.argtypes = [vp, ctypes.POINTER(ctypes.c_ulonglong)]
     L.fp_last_launch_count.argtypes = [vp, ctypes.POINTER(i)]
     for name in ("fp_create", "fp_destroy", "fp_set_option", "fp_get_option", "fp_prepare", "fp_project",
-                 "fp_project_host", "fp_ray_ranges", "fp_plan", "fp_last_sample_count", "fp_last_launch_count"):
+                 "fp_project_host", "fp_backproject", "fp_ray_ranges", "fp_plan", "fp_last_sample_count", "fp_last_launch_count"):
         getattr(L, name).restype = i
     L.fp_status_string.argtypes = [i]
     L.fp_status_string.restype = ctypes.c_char_p
@@ -181,6 +182,23 @@ class Projector:
                                             g.ctypes.data_as(ctypes.POINTER(ctypes.c_double)),
                                             int(nu), int(nv), out_host.data_ptr()))
         return out_host
+
+    def backproject(self, proj, geom, nu: int, nv: int, out=None, stream=None):
+        """fp_backproject: proj CUDA fp32 [n_proj][nv][nu] -> CUDA fp32 volume (nx,ny,nz) = A^T proj."""
+        import torch
+        g = _geom(geom)
+        n_proj = g.shape[0]
+        if not (isinstance(proj, torch.Tensor) and proj.is_cuda and proj.dtype == torch.float32 and proj.is_contiguous()
+                and proj.numel() == n_proj * nv * nu):
+            raise ValueError("proj must be a contiguous CUDA float32 tensor with n_proj*nv*nu elements")
+        if out is None:
+            out = torch.empty(self.shape, device=proj.device, dtype=torch.float32)
+        else:
+            self._check_vol(out)
+        self._check(self._L.fp_backproject(self._h, proj.data_ptr(), n_proj,
+                                           g.ctypes.data_as(ctypes.POINTER(ctypes.c_double)),
+                                           int(nu), int(nv), out.data_ptr(), _stream_handle(stream)))
+        return out
 
     def ray_ranges(self, geom, nu: int, nv: int, device="cuda", stream=None):
         """fp_ray_ranges: CUDA int32 [n_proj][nv][nu][3] = (m, i_first, i_last)."""

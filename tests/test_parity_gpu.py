@@ -433,3 +433,68 @@ def test_tma_kernel_c3_sampled_and_fallback(torch, fp, synth, oracle):
     g = out[ids[:, 0], ids[:, 1], ids[:, 2]]
     tol = 2e-5 * np.abs(ov) + 1e-6 * pl * float(np.abs(vol).max())
     assert np.all(np.abs(g - ov) <= tol), float(np.max(np.abs(g - ov) / np.maximum(tol, 1e-300)))
+
+
+# ----------------------------------------------------------------------------- back-projection
+
+def bp_tolerance(oracle, proj, shape, delta, origin, geom, kernel):
+    """|gpu - oracle| <= 2e-5 * (A^T |y|)[v] + 1e-6 * max_v (A^T 1) * max|y|: the forward tolerance transposed.
+    The relative term is taken against the sum of the magnitudes a voxel receives; the absolute term is the
+    forward's 1e-6 * path length * max|input| with the path length replaced by the largest total weight any
+    voxel receives (a voxel at the rim receives many samples with tiny weights, each carrying the same
+    absolute fp32 weight error as an interior one)."""
+    absy = oracle.backproject(np.abs(proj), shape, delta, origin, geom, kernel=kernel, threads=oracle.host_cores())
+    wsum = oracle.backproject(np.ones_like(proj), shape, delta, origin, geom, kernel=kernel, threads=oracle.host_cores())
+    return 2e-5 * absy + 1e-6 * float(wsum.max()) * float(np.abs(proj).max())
+
+
+@pytest.mark.parametrize("interp", [0, 1])
+def test_backprojection_parity_small_all_axes(torch, fp, oracle, interp):
+    rng = np.random.default_rng(500 + interp)
+    vol, delta, origin = small_problem(rng)
+    shape = vol.shape
+    nu, nv = 37, 29
+    geom = np.stack([pose(s, (0.2, -0.1, 0.3), nu, nv, 0.5, 60.0, roll)
+                     for s, roll in [((-30, 2, 1), 0.0), ((1, 28, -3), 0.4), ((2, -1, 31), 1.1),
+                                     ((-14, -15, 16), 2.0), ((20, 3, -19), 0.7)]]
+                    + [aligned_pose(0.8, 40.0, 90.0, nu, nv, 0.5), pose((-30, 200, 2), (0, 400, 0), nu, nv, 0.5, 60.0)])
+    y = rng.uniform(-1.0, 2.0, size=(len(geom), nv, nu)).astype(np.float32)
+    with fp.Projector(*shape, delta, origin) as P:
+        P.set_option(fp.OPT_INTERP, interp)
+        out = P.backproject(torch.from_numpy(y).cuda(), geom, nu, nv)
+        torch.cuda.synchronize()
+        g = out.cpu().numpy().astype(np.float64)
+        # n_proj = 0 clears the volume
+        z = P.backproject(torch.zeros((0, nv, nu), device="cuda"), np.zeros((0, 12)), nu, nv, out=out)
+        assert float(z.abs().max()) == 0.0
+    ref = oracle.backproject(y.astype(np.float64), shape, delta, origin, geom, kernel=interp, threads=oracle.host_cores())
+    tol = bp_tolerance(oracle, y.astype(np.float64), shape, delta, origin, geom, interp)
+    err = np.abs(g - ref)
+    assert np.all(err <= tol), float(np.max(err / np.maximum(tol, 1e-300)))
+    assert np.abs(ref).max() > 1.0
+
+
+def test_backprojection_c1_parity_and_adjoint_identity_at_c3_size(torch, fp, synth, oracle):
+    cfg = synth.CONFIGS["C1"]
+    geom = synth.make_geometry(cfg)
+    rng = np.random.default_rng(61)
+    y = rng.uniform(0.0, 1.0, size=(cfg.n_proj, cfg.nv, cfg.nu)).astype(np.float32)
+    with fp.Projector(*cfg.n, cfg.voxel_size, cfg.origin) as P:
+        g = P.backproject(torch.from_numpy(y).cuda(), geom, cfg.nu, cfg.nv).cpu().numpy().astype(np.float64)
+    ref = oracle.backproject(y.astype(np.float64), cfg.n, cfg.voxel_size, cfg.origin, geom, threads=oracle.host_cores())
+    tol = bp_tolerance(oracle, y.astype(np.float64), cfg.n, cfg.voxel_size, cfg.origin, geom, 0)
+    assert np.all(np.abs(g - ref) <= tol)
+    # a property that holds at any size: <A x, y> = <x, A^T y> with the (oracle-checked) forward kernel,
+    # on the full 512^3 volume and four C3 poses
+    cfg = synth.CONFIGS["C3"]
+    geom = synth.make_geometry(cfg)[[3, 47, 200, 311]]
+    x = synth.make_volume(cfg, device="cuda")
+    gen = torch.Generator(device="cuda").manual_seed(5)
+    yy = torch.rand((len(geom), cfg.nv, cfg.nu), device="cuda", generator=gen)
+    with fp.Projector(*cfg.n, cfg.voxel_size, cfg.origin) as P:
+        ax = P.project(x, geom, cfg.nu, cfg.nv)
+        aty = P.backproject(yy, geom, cfg.nu, cfg.nv)
+        torch.cuda.synchronize()
+    lhs = float((ax.double() * yy.double()).sum())
+    rhs = float((x.double() * aty.double()).sum())
+    assert abs(lhs - rhs) <= 2e-5 * abs(lhs), (lhs, rhs)
