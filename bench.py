@@ -183,6 +183,54 @@ def workload_name(cfg):
         cfg.name, *cfg.n, cfg.n_proj, cfg.orbit, cfg.nu, cfg.nv)
 
 
+def run_backproject(args, torch, fp, cfg, geom, vol, proj, P, stream, world, rank, dist):
+    """--op backproject: one step = fp_backproject of the whole orbit (A^T applied to the projections of the
+    synthetic volume) into a volume-sized output; reported as back-projected projections per second."""
+    P.project(vol, geom, cfg.nu, cfg.nv, out=proj, stream=stream)          # the input: A x
+    bp = torch.empty_like(vol)
+
+    def step():
+        P.backproject(proj, geom, cfg.nu, cfg.nv, out=bp, stream=stream)
+        return P.last_launch_count()
+
+    for _ in range(args.warmup):
+        step()
+    torch.cuda.synchronize()
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps + 1)]
+    clocks = ClockSampler(int(os.environ.get("LOCAL_RANK", "0")))
+    time.sleep(0.25)
+    launches = 0
+    ev[0].record(stream)
+    for k in range(args.steps):
+        launches += step()
+        ev[k + 1].record(stream)
+    torch.cuda.synchronize()
+    clk = clocks.stop()
+    ms = max_over_ranks(dist, ev[0].elapsed_time(ev[args.steps])) / args.steps
+    if rank != 0:
+        return 0
+    # adjoint identity on the timed data: <A x, A x> = <x, A^T A x>
+    lhs = float((proj.double() ** 2).sum())
+    rhs = float((vol.double() * bp.double()).sum())
+    peaks, peak_kind = measured_peaks()
+    vol_bytes, proj_bytes = vol.numel() * 4, cfg.nu * cfg.nv * 4
+    algo = cfg.n_proj * (2 * vol_bytes + proj_bytes)        # read-modify-write of the volume once per projection
+    achieved = algo / (ms * 1e-3) / 1e9
+    line = {
+        "metric": "512^3 cone-beam back-projections/s", "value": replicas_throughput(world, cfg.n_proj, ms * 1e-3),
+        "unit": "projections/s", "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "config": {"workload": workload_name(cfg), "op": "backproject", "interpolation": args.interp},
+        "clocks": clk, "gpu_launches": launches,
+        "roofline": {"bound": "hbm", "achieved": achieved, "peak": peaks["hbm_gbs"], "unit": "GB/s",
+                     "frac": achieved / peaks["hbm_gbs"], "traffic": None, "peak_kind": peak_kind,
+                     "kernel": "fp_backproject_kernel", "algorithmic_bytes_per_launch": algo},
+        "adjoint_check": {"lhs": lhs, "rhs": rhs, "rel_diff": abs(lhs - rhs) / abs(lhs)},
+    }
+    print(json.dumps(line))
+    return 0
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -193,6 +241,8 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--kernel", type=int, default=0, help="FP_OPT_KERNEL value (0 = auto)")
+    ap.add_argument("--op", default="project", choices=["project", "backproject"],
+                    help="project: the headline forward projector; backproject: its exact transpose (SURVEY 8(f) #2)")
     ap.add_argument("--interp", default="linear", choices=["linear", "spline"],
                     help="interpolation kernel: GJP_lin (PAPER.md:150 Eq. 13, the headline) or GJP_spl (:152 Eq. 14)")
     args = ap.parse_args()
@@ -226,6 +276,9 @@ def main():
     interp = fp.INTERP_SPLINE if args.interp == "spline" else fp.INTERP_LINEAR
     P.set_option(fp.OPT_INTERP, interp)
     stream = torch.cuda.current_stream()
+
+    if args.op == "backproject":
+        return run_backproject(args, torch, fp, cfg, geom, vol, out, P, stream, world, rank, dist)
 
     def step():
         launches, samples = 0, None
