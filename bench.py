@@ -355,8 +355,16 @@ def main():
         return 0
 
     # which sampling kernel the library's plan picks for this workload (fp_plan, host only)
-    kernel_name = {fp.KERNEL_DIRECT: "fp_direct_kernel", fp.KERNEL_ALIGNED: "fp_aligned_kernel",
-                   fp.KERNEL_TMA: "fp_tma_kernel"}[P.plan(geom[0], cfg.nu, cfg.nv)[0]]
+    # (a call's aligned poses go to the TMA-fed kernel only if ALL of them fit its tile)
+    plans = {P.plan(g, cfg.nu, cfg.nv)[0] for g in geom[:batch]}
+    if plans == {fp.KERNEL_TMA}:
+        kernel_name = "fp_tma_kernel"
+    elif plans <= {fp.KERNEL_TMA, fp.KERNEL_ALIGNED}:
+        kernel_name = "fp_aligned_kernel"
+    elif plans == {fp.KERNEL_DIRECT}:
+        kernel_name = "fp_direct_kernel"
+    else:
+        kernel_name = "fp_direct_kernel + fp_aligned_kernel"
     peaks, peak_kind = measured_peaks()
     vol_bytes = vol.numel() * 4
     out_bytes_per_proj = cfg.nu * cfg.nv * 4
