@@ -38,7 +38,7 @@ struct fp_ctx {
     int ids_cap = 0;
     bool aligned_attr_set = false;
     // tensor maps of the TMA kernel: valid for one volume pointer
-    CUtensorMap tmap[2][kTmMaps];
+    CUtensorMap tmap[2][kTmWBoxes][kTmMaps];
     const float *tmap_vol = nullptr;
     cudaStream_t last_stream = nullptr;
     bool counted = false;
@@ -364,18 +364,19 @@ static fp_status build_tensor_maps(fp_ctx *c, const float *vol)
     const cuuint64_t strides[2] = {(cuuint64_t)c->G.n[2] * 4, (cuuint64_t)c->G.n[2] * c->G.n[1] * 4};
     const cuuint32_t estr[3] = {1, 1, 1};
     for (int pass = 0; pass < 2; ++pass)
-        for (int big = 0; big < kTmMaps; ++big) {
-            const cuuint32_t rows = 4 + 2 * big;
-            const cuuint32_t box[3] = {(cuuint32_t)kTmW, pass == 0 ? rows : 1u, pass == 0 ? 1u : rows};
-            const CUresult r = encode(&c->tmap[pass][big], CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, (void *)vol, dims, strides, box,
-                                      estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
-                                      CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-            if (r != CUDA_SUCCESS) {
-                char buf[96];
-                snprintf(buf, sizeof buf, "cuTensorMapEncodeTiled failed (%d)", (int)r);
-                return fail(c, FP_ERR_CUDA, buf);
+        for (int wi = 0; wi < kTmWBoxes; ++wi)
+            for (int big = 0; big < kTmMaps; ++big) {
+                const cuuint32_t rows = 4 + 2 * big, width = kTmWMin + kTmWStep * wi;
+                const cuuint32_t box[3] = {width, pass == 0 ? rows : 1u, pass == 0 ? 1u : rows};
+                const CUresult r = encode(&c->tmap[pass][wi][big], CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, (void *)vol, dims,
+                                          strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                                          CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+                if (r != CUDA_SUCCESS) {
+                    char buf[96];
+                    snprintf(buf, sizeof buf, "cuTensorMapEncodeTiled failed (%d)", (int)r);
+                    return fail(c, FP_ERR_CUDA, buf);
+                }
             }
-        }
     c->tmap_vol = vol;
     return FP_OK;
 }

@@ -26,13 +26,15 @@ constexpr int kTmSB = 4;                 // slices per batch = pipeline stages
 constexpr int kTmRows = 256;             // detector rows per block, two per consumer thread
 constexpr int kTmConsumers = kTmRows / 2;
 constexpr int kTmThreads = kTmConsumers + 32;
-constexpr int kTmW = 256;                // z window (voxels) = inner TMA box size
+constexpr int kTmW = 256;                // largest z window (voxels) = largest inner TMA box size
+constexpr int kTmWBoxes = 4;             // inner box sizes 160, 192, 224, 256: the tile's row pitch follows the box
+constexpr int kTmWMin = 160, kTmWStep = 32;
 constexpr int kTmNR = 12;                // volume rows per tile (largest box); two zero rows follow
 constexpr int kTmMaps = 5;                // tensor maps per pass: boxes of 4, 6, 8, 10, 12 rows
 constexpr int kTmStageFloats = kTmNR * kTmW;   // the stages are followed by two zero rows shared by all of them
 
 struct __align__(64) TmaParams {
-    CUtensorMap map[2][kTmMaps];       // [pass = driving axis x / y][box of 4, 6, 8, 10 or 12 rows]
+    CUtensorMap map[2][kTmWBoxes][kTmMaps];   // [pass = driving axis x / y][box width][box of 4, 6, 8, 10 or 12 rows]
     GridDesc G;
     const ProjDesc *proj;              // all projections of the call
     const int *ids;                    // [n_sel] projections this launch handles
@@ -53,6 +55,7 @@ struct __align__(16) TmShared {
     uint2 stage_col[kTmSB][kTmTU];     // per (stage, column): byte offset of its lower row in the tile, weight bits
     double t0[2][kTmTU];               // per (batch parity, column): (i0 - s_m) / r_m
     double off[2];                     // per batch parity: s_z - z0
+    unsigned pitch[2];                 // per batch parity: byte pitch of the tile rows (= box width * 4)
     TmColumn col[kTmTU];
     double s[3];                       // source, grid units
     double rxy[kTmTU][2];              // r_x, r_y per column
@@ -196,15 +199,22 @@ __device__ __forceinline__ void tm_produce_batch(TmShared &S, const TmaParams &P
     const int zhi = __reduce_max_sync(0xffffffffu, al_to_int(floor(fmax(za, zb))));
     // taps k, k+1 with k = floor(p_z - z0) in [1, W-3] (one spare on either side for fp32 rounding)
     const int z0 = (zlo - 1) & ~3;
-    const bool winok = (zlo > -1000000000) && (zhi < 1000000000) && (zhi + 3 - z0 <= kTmW);
+    const int need = zhi + 3 - z0;
+    const bool winok = (zlo > -1000000000) && (zhi < 1000000000) && (need <= kTmW);
+    // narrowest box that holds the window: less HBM / L2 / shared-memory traffic than always copying 256 voxels
+    const int wi = winok ? min(max((need - kTmWMin + kTmWStep - 1) / kTmWStep, 0), kTmWBoxes - 1) : kTmWBoxes - 1;
+    const int pitch = kTmWMin + kTmWStep * wi;
     if (!winok && lane == 0) atomicOr(P.err_flag, 1u);
     const int par = gb & 1;
     if (s == 0) S.t0[par][c] = winok ? __dmul_rn(__dsub_rn((double)i0, S.s_m), C.inv_rm) : 0.0;
     // a window that does not fit is never sampled out of bounds: park every row at p = 4
-    if (lane == 0) S.off[par] = winok ? S.s[2] - (double)z0 : 4.0;
+    if (lane == 0) {
+        S.off[par] = winok ? S.s[2] - (double)z0 : 4.0;
+        S.pitch[par] = (unsigned)(pitch * 4);
+    }
     uint2 pc;
     // a column without a sample on this slice reads the two zero rows behind the last stage
-    pc.x = (fits && winok) ? (unsigned)((j - jmin) * kTmW * 4) : (unsigned)((kTmSB - s) * kTmStageFloats * 4);
+    pc.x = (fits && winok) ? (unsigned)((j - jmin) * pitch * 4) : (unsigned)((kTmSB - s) * kTmStageFloats * 4);
     pc.y = (fits && winok) ? __float_as_uint(u) : 0u;
 #pragma unroll
     for (int ss = 0; ss < kTmSB; ++ss) {
@@ -218,8 +228,8 @@ __device__ __forceinline__ void tm_produce_batch(TmShared &S, const TmaParams &P
         __syncwarp();
         if (lane == 0) {
             if (al_s && winok) {
-                tm_mbar_arrive_tx(&S.full[ss], (unsigned)((4 + 2 * mi_s) * kTmW * 4));
-                const CUtensorMap *map = &P.map[pass][mi_s];
+                tm_mbar_arrive_tx(&S.full[ss], (unsigned)((4 + 2 * mi_s) * pitch * 4));
+                const CUtensorMap *map = &P.map[pass][wi][mi_s];
                 // tensor dimensions are (z, y, x); the slow axis is y for m = x and x for m = y
                 if (pass == 0)
                     tm_load_3d(map, tiles + ss * kTmStageFloats, &S.full[ss], z0, jmin_s, i_s);
@@ -308,8 +318,10 @@ fp_tma_kernel(const __grid_constant__ TmaParams P)
                 const unsigned par = gb & 1;
                 tm_mbar_wait(&S.full[0], par);
                 float2 a[kTmTU];
+                unsigned pitchB;
                 {
                     const double off = S.off[par];
+                    pitchB = S.pitch[par];
 #pragma unroll
                     for (int c = 0; c < kTmTU; ++c) {
                         const double t0 = S.t0[par][c];
@@ -335,8 +347,9 @@ fp_tma_kernel(const __grid_constant__ TmaParams P)
                         const unsigned a0 = (__float_as_uint(x.x) << 2) + rb, a1 = (__float_as_uint(x.y) << 2) + rb;
                         const float2 v00 = make_float2(al_lds(a0), al_lds(a1));
                         const float2 v01 = make_float2(al_lds(a0 + 4u), al_lds(a1 + 4u));
-                        const float2 v10 = make_float2(al_lds(a0 + kTmW * 4u), al_lds(a1 + kTmW * 4u));
-                        const float2 v11 = make_float2(al_lds(a0 + kTmW * 4u + 4u), al_lds(a1 + kTmW * 4u + 4u));
+                        const unsigned b0 = a0 + pitchB, b1 = a1 + pitchB;        // row j + 1
+                        const float2 v10 = make_float2(al_lds(b0), al_lds(b1));
+                        const float2 v11 = make_float2(al_lds(b0 + 4u), al_lds(b1 + 4u));
                         const float2 wz = make_float2(ceil_weight<INTERP>(d.x), ceil_weight<INTERP>(d.y));
                         const float uy = __uint_as_float(pc.y);
                         const float2 t0 = __ffma2_rn(wz, __ffma2_rn(v00, kNegOne2, v01), v00);   // row j
