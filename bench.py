@@ -33,7 +33,7 @@ TAP_BYTES = 16           # 4 taps x 4 B per sample: the paper's "memory access r
 FALLBACK_HBM_GBS = 6650.0
 # dram__bytes_read.sum + dram__bytes_write.sum of one launch, from the committed ncu --set full captures
 # (profiles/r1_02_aligned_kernel_c3.md, profiles/r1_03_tma_kernel_c3.md); None where no capture exists
-NCU_TRAFFIC_BYTES = {("C3", "fp_aligned_kernel"): 201.51e9, ("C3", "fp_tma_kernel"): 273.31e9}
+NCU_TRAFFIC_BYTES = {("C3", "fp_aligned_kernel"): 201.51e9, ("C3", "fp_tma_kernel"): 223.54e9}
 
 
 def measured_peaks():
