@@ -498,3 +498,27 @@ def test_backprojection_c1_parity_and_adjoint_identity_at_c3_size(torch, fp, syn
     lhs = float((ax.double() * yy.double()).sum())
     rhs = float((x.double() * aty.double()).sum())
     assert abs(lhs - rhs) <= 2e-5 * abs(lhs), (lhs, rhs)
+
+
+def test_tma_kernel_follows_the_volume_pointer_and_contents(torch, fp, oracle):
+    """The tensor maps of the TMA-fed kernel are cached per volume pointer: a second volume at another address
+    and new contents at the same address must both be projected from the data as it is at call time."""
+    rng = np.random.default_rng(77)
+    shape, delta = (24, 20, 32), 0.9
+    origin = tuple(-(n - 1) / 2.0 * delta for n in shape)
+    nu, nv = 40, 36
+    geom = np.stack([aligned_pose(th, 50.0, 110.0, nu, nv, 0.8) for th in (0.3, 1.9, 4.0)])
+    ids = all_ids(len(geom), nv, nu)
+    va = rng.uniform(0.0, 1.0, size=shape).astype(np.float32)
+    vb = rng.uniform(-1.0, 1.0, size=shape).astype(np.float32)
+    ta, tb = torch.from_numpy(va).cuda(), torch.from_numpy(vb).cuda()
+    with fp.Projector(*shape, delta, origin) as P:
+        assert all(P.plan(g, nu, nv)[0] == fp.KERNEL_TMA for g in geom)
+        outs = [P.project(ta, geom, nu, nv).cpu().numpy(), P.project(tb, geom, nu, nv).cpu().numpy()]
+        ta.copy_(tb)                                       # same pointer, new contents
+        outs.append(P.project(ta, geom, nu, nv).cpu().numpy())
+        mfl = P.ray_ranges(geom, nu, nv).cpu().numpy()
+    for out, v in zip(outs, (va, vb, vb)):
+        ov, om, pl, mg = oracle.project_rays(v, delta, origin, geom, ids)
+        assert assert_parity(out.ravel(), mfl.reshape(-1, 3), ov, om, pl, mg, float(np.abs(v).max())) < 1.0
+    assert np.array_equal(outs[1], outs[2])
