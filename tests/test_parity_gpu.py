@@ -522,3 +522,23 @@ def test_tma_kernel_follows_the_volume_pointer_and_contents(torch, fp, oracle):
         ov, om, pl, mg = oracle.project_rays(v, delta, origin, geom, ids)
         assert assert_parity(out.ravel(), mfl.reshape(-1, 3), ov, om, pl, mg, float(np.abs(v).max())) < 1.0
     assert np.array_equal(outs[1], outs[2])
+
+
+@pytest.mark.parametrize("kernel_opt", ["tma", "aligned"])
+def test_aligned_class_kernels_on_degenerate_grids_and_detectors(torch, fp, oracle, kernel_opt):
+    """One-voxel-thick volumes along x or y, the smallest z extent the float4 / TMA paths take (nz = 4),
+    1 x 1 and 1 x n detectors, poses on the axes and on the diagonals."""
+    rng = np.random.default_rng(88)
+    opt = fp.KERNEL_TMA if kernel_opt == "tma" else fp.KERNEL_ALIGNED
+    for shape in [(1, 9, 8), (9, 1, 8), (5, 6, 4), (2, 2, 12)]:
+        vol = rng.uniform(0.5, 1.5, size=shape).astype(np.float32)
+        origin = tuple(-(n - 1) / 2.0 for n in shape)
+        for nu, nv in [(1, 1), (1, 7), (9, 1), (12, 10)]:
+            geom = np.stack([aligned_pose(th, 30.0, 60.0, nu, nv, 0.7, src_z=0.4)
+                             for th in (0.0, math.pi / 4, math.pi / 2, 2.2, math.pi, 5.4977871)])
+            with fp.Projector(*shape, 1.0, origin) as P:
+                P.set_option(fp.OPT_KERNEL, opt)
+                assert all(P.plan(g, nu, nv)[0] == opt for g in geom), (shape, nu, nv)
+            worst, _, _ = compare_full(torch, fp, oracle, vol, 1.0, origin, geom, nu, nv,
+                                       options=[(fp.OPT_KERNEL, opt)], what="%s %s %dx%d" % (kernel_opt, shape, nu, nv))
+            assert worst < 1.0
