@@ -48,7 +48,9 @@ struct fp_ctx {
     float *hout_dev[2] = {nullptr, nullptr};
     size_t hout_cap = 0;
     cudaStream_t hstream[2] = {nullptr, nullptr};
-    cudaEvent_t hevent[2] = {nullptr, nullptr};
+    cudaEvent_t hevent[2] = {nullptr, nullptr};      // batch sampled (compute stream)
+    cudaEvent_t hcopied[2] = {nullptr, nullptr};     // batch copied to the host (copy stream)
+    bool keep_count = false;                         // fp_project_host: batches add to one sample count
     std::string err;
 };
 
@@ -124,6 +126,7 @@ extern "C" fp_status fp_destroy(fp_ctx *c)
         cudaFree(c->hout_dev[k]);
         if (c->hstream[k]) cudaStreamDestroy(c->hstream[k]);
         if (c->hevent[k]) cudaEventDestroy(c->hevent[k]);
+        if (c->hcopied[k]) cudaEventDestroy(c->hcopied[k]);
     }
     cudaGetLastError();
     delete c;
@@ -521,7 +524,7 @@ extern "C" fp_status fp_project(fp_ctx *c, const float *vol_dev, int n_proj, con
                                    cudaMemcpyHostToDevice, st));
 
     if (!c->count_dev) FP_CUDA(c, cudaMalloc(&c->count_dev, 2 * sizeof(unsigned long long)));
-    FP_CUDA(c, cudaMemsetAsync(c->count_dev, 0, 2 * sizeof(unsigned long long), st));
+    if (!c->keep_count) FP_CUDA(c, cudaMemsetAsync(c->count_dev, 0, 2 * sizeof(unsigned long long), st));
     c->counted = c->opt_count != 0;
 
     if (!ids_al.empty() && c->opt_kernel != FP_KERNEL_ALIGNED && w_al <= kTmW && rows_al <= kTmNR) {
@@ -694,44 +697,49 @@ extern "C" fp_status fp_project_host(fp_ctx *c, const float *vol_host, int n_pro
         }
         c->hout_cap = (size_t)batch * per_proj;
     }
-    FP_CUDA(c, cudaMemcpyAsync(c->hvol_dev, vol_host, nvox * sizeof(float), cudaMemcpyHostToDevice, c->hstream[0]));
-    FP_CUDA(c, cudaEventRecord(c->hevent[0], c->hstream[0]));
-    FP_CUDA(c, cudaStreamWaitEvent(c->hstream[1], c->hevent[0], 0));
+    for (int k = 0; k < 2; ++k)
+        if (!c->hcopied[k]) FP_CUDA(c, cudaEventCreateWithFlags(&c->hcopied[k], cudaEventDisableTiming));
+    // stream 0 carries the volume upload and every kernel, stream 1 the device-to-host copies: the copy of
+    // batch k overlaps the kernels of batch k+1, and the host plans batch k+1 while batch k runs (no host
+    // synchronisation inside the loop; the shared geometry buffer is safe because all kernels are in one stream)
+    cudaStream_t compute = c->hstream[0], copy = c->hstream[1];
+    FP_CUDA(c, cudaMemcpyAsync(c->hvol_dev, vol_host, nvox * sizeof(float), cudaMemcpyHostToDevice, compute));
+    if (!c->count_dev) FP_CUDA(c, cudaMalloc(&c->count_dev, 2 * sizeof(unsigned long long)));
+    FP_CUDA(c, cudaMemsetAsync(c->count_dev, 0, 2 * sizeof(unsigned long long), compute));
     // the layout copy (if any) is made once, then kept for all batches
     const int was_volatile = c->opt_volatile;
-    unsigned long long total = 0;
     int launches = 0;
-    bool first = true;
+    c->keep_count = true;
     for (int p0 = 0, b = 0; p0 < n_proj; p0 += batch, ++b) {
         const int k = b & 1;
         const int np = std::min(batch, n_proj - p0);
-        if (!first) c->opt_volatile = 0;
-        // each batch's kernel has finished (host sync below) before the next batch is planned, so the
-        // shared geometry buffer is free; only the device-to-host copies overlap the next kernels
-        s = fp_project(c, c->hvol_dev, np, geom + 12 * (size_t)p0, nu, nv, c->hout_dev[k], c->hstream[k]);
+        if (b > 0) c->opt_volatile = 0;
+        cudaError_t e = b >= 2 ? cudaStreamWaitEvent(compute, c->hcopied[k], 0) : cudaSuccess;   // output buffer k is free
+        s = e == cudaSuccess ? fp_project(c, c->hvol_dev, np, geom + 12 * (size_t)p0, nu, nv, c->hout_dev[k], compute)
+                             : cuda_fail(c, e, "cudaStreamWaitEvent");
         c->opt_volatile = was_volatile;
-        if (s != FP_OK) return s;
-        launches += c->last_launches;
-        first = false;
-        if (c->opt_count) {
-            unsigned long long n = 0;
-            s = fp_last_sample_count(c, &n);      // synchronises this batch's stream
-            if (s != FP_OK) return s;
-            total += n;
-        } else {
-            FP_CUDA(c, cudaStreamSynchronize(c->hstream[k]));
+        if (s == FP_OK) {
+            launches += c->last_launches;
+            e = cudaEventRecord(c->hevent[k], compute);
+            if (e == cudaSuccess) e = cudaStreamWaitEvent(copy, c->hevent[k], 0);
+            if (e == cudaSuccess)
+                e = cudaMemcpyAsync(out_host + (size_t)p0 * per_proj, c->hout_dev[k], (size_t)np * per_proj * sizeof(float),
+                                    cudaMemcpyDeviceToHost, copy);
+            if (e == cudaSuccess) e = cudaEventRecord(c->hcopied[k], copy);
+            if (e != cudaSuccess) s = cuda_fail(c, e, "fp_project_host: copy pipeline");
         }
-        FP_CUDA(c, cudaMemcpyAsync(out_host + (size_t)p0 * per_proj, c->hout_dev[k], (size_t)np * per_proj * sizeof(float),
-                                   cudaMemcpyDeviceToHost, c->hstream[k]));
+        if (s != FP_OK) {
+            c->keep_count = false;
+            cudaStreamSynchronize(compute);
+            cudaStreamSynchronize(copy);
+            return s;
+        }
     }
-    FP_CUDA(c, cudaStreamSynchronize(c->hstream[0]));
-    FP_CUDA(c, cudaStreamSynchronize(c->hstream[1]));
+    c->keep_count = false;
+    FP_CUDA(c, cudaStreamSynchronize(compute));
+    FP_CUDA(c, cudaStreamSynchronize(copy));
     c->last_launches = launches;
-    if (c->opt_count) {
-        // leave the total where fp_last_sample_count finds it
-        FP_CUDA(c, cudaMemcpy(c->count_dev, &total, sizeof total, cudaMemcpyHostToDevice));
-        c->last_stream = c->hstream[0];
-        c->counted = true;
-    }
+    c->last_stream = compute;
+    c->counted = c->opt_count != 0;
     return FP_OK;
 }
