@@ -236,7 +236,7 @@ def main():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--config", default="C3", choices=["C1", "C2", "C3", "C4", "C5"])
+    ap.add_argument("--config", default="C3", choices=["C1", "C2", "C3", "C4", "C5", "P1"])
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
@@ -355,16 +355,11 @@ def main():
         return 0
 
     # which sampling kernel the library's plan picks for this workload (fp_plan, host only)
-    # (a call's aligned poses go to the TMA-fed kernel only if ALL of them fit its tile)
-    plans = {P.plan(g, cfg.nu, cfg.nv)[0] for g in geom[:batch]}
-    if plans == {fp.KERNEL_TMA}:
-        kernel_name = "fp_tma_kernel"
-    elif plans <= {fp.KERNEL_TMA, fp.KERNEL_ALIGNED}:
-        kernel_name = "fp_aligned_kernel"
-    elif plans == {fp.KERNEL_DIRECT}:
-        kernel_name = "fp_direct_kernel"
-    else:
-        kernel_name = "fp_direct_kernel + fp_aligned_kernel"
+    plans = [P.plan(g, cfg.nu, cfg.nv)[0] for g in geom]
+    names = {fp.KERNEL_DIRECT: "fp_direct_kernel", fp.KERNEL_ALIGNED: "fp_aligned_kernel", fp.KERNEL_TMA: "fp_tma_kernel"}
+    # every pose is planned on its own; name the kernel that takes most of them and say how many
+    kernel_name = names[max(set(plans), key=plans.count)]
+    kernel_share = {names[k]: plans.count(k) for k in sorted(set(plans))}
     peaks, peak_kind = measured_peaks()
     vol_bytes = vol.numel() * 4
     out_bytes_per_proj = cfg.nu * cfg.nv * 4
@@ -374,7 +369,7 @@ def main():
     achieved = algo_bytes_per_step / (kernel_ms * 1e-3) / 1e9
     roofline = {"bound": "hbm", "achieved": achieved, "peak": peaks["hbm_gbs"], "unit": "GB/s",
                 "frac": achieved / peaks["hbm_gbs"], "traffic": NCU_TRAFFIC_BYTES.get((cfg.name, kernel_name)), "peak_kind": peak_kind,
-                "kernel": kernel_name, "algorithmic_bytes_per_launch": algo_bytes_per_step // max(1, (cfg.n_proj + batch - 1) // batch)}
+                "kernel": kernel_name, "projections_per_kernel": kernel_share, "algorithmic_bytes_per_launch": algo_bytes_per_step // max(1, (cfg.n_proj + batch - 1) // batch)}
 
     cpu_baseline = None
     parity = None

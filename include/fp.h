@@ -65,8 +65,8 @@ enum {
     /* Sampling-kernel variant.  Poses whose v vector is parallel to the volume's z axis, whose u vector is
      * perpendicular to it and that have no z-driven ray (every circular orbit about z)
      * are "aligned"; all other poses always use FP_KERNEL_DIRECT (one thread per ray, four global taps per
-     * sample).  For the aligned poses of a call:
-     *   FP_KERNEL_AUTO     FP_KERNEL_TMA if they all fit a 256-voxel z window and 12 volume rows per block
+     * sample).  For each aligned pose (one launch per kernel and call):
+     *   FP_KERNEL_AUTO     FP_KERNEL_TMA if the pose fits a 256-voxel z window and 12 volume rows per block
      *                      and slice, else FP_KERNEL_ALIGNED;
      *   FP_KERNEL_TMA      the same as AUTO (tiles of the caller's volume copied to shared memory by
      *                      cp.async.bulk.tensor, four taps per sample read from the tile);
@@ -166,8 +166,8 @@ fp_status fp_last_sample_count(fp_ctx *ctx, unsigned long long *n);
 
 /*
  * fp_plan: the host-side plan fp_project makes for ONE pose (no device needed, nothing is launched):
- *   *kernel    FP_KERNEL_ALIGNED, FP_KERNEL_TMA or FP_KERNEL_DIRECT: the sampling kernel a call with this
- *              pose alone would use under the current FP_OPT_KERNEL
+ *   *kernel    FP_KERNEL_ALIGNED, FP_KERNEL_TMA or FP_KERNEL_DIRECT: the sampling kernel this pose gets
+ *              under the current FP_OPT_KERNEL
  *   *window    staging window of the aligned kernel in voxels along z (0 for the direct kernel)
  *   *z_driven  1 if some ray of the pose has z as its driving axis (Eq. 2), which is
  *              what makes fp_project build the permuted copy of the layout stage

@@ -34,7 +34,7 @@ struct fp_ctx {
     ProjDesc *proj_dev = nullptr;
     int proj_cap = 0;
     unsigned long long *count_dev = nullptr;   // [0] sample count, [1] (low word) staging-window error flag
-    int *ids_dev = nullptr;                    // [2 * ids_cap]: aligned ids, then direct ids
+    int *ids_dev = nullptr;                    // [3 * ids_cap]: aligned ids, direct ids, TMA ids
     int ids_cap = 0;
     bool aligned_attr_set = false;
     // tensor maps of the TMA kernel: valid for one volume pointer
@@ -316,7 +316,7 @@ static fp_status ensure_ids(fp_ctx *c, int n_proj)
         c->ids_cap = 0;
     }
     const int cap = n_proj + 64;
-    FP_CUDA(c, cudaMalloc(&c->ids_dev, sizeof(int) * 2 * (size_t)cap));
+    FP_CUDA(c, cudaMalloc(&c->ids_dev, sizeof(int) * 3 * (size_t)cap));
     c->ids_cap = cap;
     return FP_OK;
 }
@@ -488,15 +488,16 @@ extern "C" fp_status fp_project(fp_ctx *c, const float *vol_dev, int n_proj, con
     if (n_proj == 0) return FP_OK;
 
     // plan: which kernel takes which projection
-    std::vector<int> ids_al, ids_di;
-    int w_al = 0, rows_al = 0;
+    std::vector<int> ids_al, ids_di, ids_tm;
+    int w_al = 0;
     for (int p = 0; p < n_proj; ++p) {
         int rows = 0;
         const int w = c->opt_kernel == FP_KERNEL_DIRECT ? 0 : plan_aligned(c, vol_dev, geom + 12 * (size_t)p, nu, nv, &rows);
-        if (w > 0 && w <= kAlignedMaxW) {
+        if (w > 0 && w <= kTmW && rows <= kTmNR && c->opt_kernel != FP_KERNEL_ALIGNED) {
+            ids_tm.push_back(p);                       // fits the TMA-fed kernel's tile
+        } else if (w > 0 && w <= kAlignedMaxW) {
             ids_al.push_back(p);
             w_al = std::max(w_al, w);
-            rows_al = std::max(rows_al, rows);
         } else {
             ids_di.push_back(p);
         }
@@ -522,30 +523,34 @@ extern "C" fp_status fp_project(fp_ctx *c, const float *vol_dev, int n_proj, con
     if (!ids_di.empty())
         FP_CUDA(c, cudaMemcpyAsync(c->ids_dev + c->ids_cap, ids_di.data(), sizeof(int) * ids_di.size(),
                                    cudaMemcpyHostToDevice, st));
+    if (!ids_tm.empty())
+        FP_CUDA(c, cudaMemcpyAsync(c->ids_dev + 2 * c->ids_cap, ids_tm.data(), sizeof(int) * ids_tm.size(),
+                                   cudaMemcpyHostToDevice, st));
 
     if (!c->count_dev) FP_CUDA(c, cudaMalloc(&c->count_dev, 2 * sizeof(unsigned long long)));
     if (!c->keep_count) FP_CUDA(c, cudaMemsetAsync(c->count_dev, 0, 2 * sizeof(unsigned long long), st));
     c->counted = c->opt_count != 0;
 
-    if (!ids_al.empty() && c->opt_kernel != FP_KERNEL_ALIGNED && w_al <= kTmW && rows_al <= kTmNR) {
+    if (!ids_tm.empty()) {
         s = build_tensor_maps(c, vol_dev);
         if (s != FP_OK) return s;
         TmaParams T;
         memcpy(T.map, c->tmap, sizeof T.map);
         T.G = c->G;
         T.proj = c->proj_dev;
-        T.ids = c->ids_dev;
+        T.ids = c->ids_dev + 2 * c->ids_cap;
         T.out = out_dev;
         T.sample_count = c->opt_count ? c->count_dev : nullptr;
         T.err_flag = reinterpret_cast<unsigned int *>(c->count_dev + 1);
         T.nu = nu;
         T.nv = nv;
-        T.n_sel = (int)ids_al.size();
-        dim3 grid((unsigned)((nu + kTmTU - 1) / kTmTU), (unsigned)((nv + kTmRows - 1) / kTmRows), (unsigned)ids_al.size());
+        T.n_sel = (int)ids_tm.size();
+        dim3 grid((unsigned)((nu + kTmTU - 1) / kTmTU), (unsigned)((nv + kTmRows - 1) / kTmRows), (unsigned)ids_tm.size());
         s = c->opt_interp == FP_INTERP_SPLINE ? launch_tma<1>(c, T, grid, st) : launch_tma<0>(c, T, grid, st);
         if (s != FP_OK) return s;
         c->last_launches += 1;
-    } else if (!ids_al.empty()) {
+    }
+    if (!ids_al.empty()) {
         AlignedParams A;
         A.G = c->G;
         A.vol = vol_dev;

@@ -72,6 +72,12 @@ CONFIGS = {
                  "random", 256, 600.0, 900.0, 1024, 1024, 1.25),
     "C5": Config("C5", 5, (1024, 1024, 1024), 0.5, 60, (10.0, 150.0), "gauss", 0.01,
                  "circular", 720, 800.0, 1200.0, 1536, 1536, 0.6, batch=64),
+    # Paper-shaped workload (SURVEY.md 8(f) #4; PAPER.md:312 sec. 3.2, :283 Eq. 17): 512^3 box, 512^2 detector,
+    # 10 degree full cone, 360 angles, grid matched by Eq. 17 (voxel pitch 1): S = 256 / sin 5deg, D = S / 2,
+    # detector pitch (S + D) tan 5deg / 256.  Not a BASELINE.json config; the volume is the C3 phantom (the
+    # paper's cylinder data is not available) and rays are not clipped to a cylinder.
+    "P1": Config("P1", 6, (512, 512, 512), 1.0, 40, (10.0, 160.0), "gauss", 0.01,
+                 "circular", 360, 2937.2705908915, 4405.9058863372, 512, 512, 1.5057297563),
 }
 
 

@@ -17,7 +17,7 @@ def circular_pose(theta, sid, sdd, nu, nv, pitch):
     return np.concatenate([S, C - (nu - 1) / 2 * U - (nv - 1) / 2 * V, U, V])
 
 
-@pytest.mark.parametrize("name,wmax", [("C1", 128), ("C2", 256), ("C3", 256), ("C5", 384)])
+@pytest.mark.parametrize("name,wmax", [("C1", 128), ("C2", 256), ("C3", 256), ("C5", 384), ("P1", 384)])
 def test_circular_orbits_take_the_aligned_kernel(name, wmax):
     cfg = synth.CONFIGS[name]
     geom = synth.make_geometry(cfg)
