@@ -275,6 +275,8 @@ def main():
         P.set_option(fp.OPT_KERNEL, args.kernel)
     interp = fp.INTERP_SPLINE if args.interp == "spline" else fp.INTERP_LINEAR
     P.set_option(fp.OPT_INTERP, interp)
+    if cfg.cylinder:
+        P.set_option(fp.OPT_FOV_CYLINDER, 1)       # the volume is zero outside the inscribed cylinder
     stream = torch.cuda.current_stream()
 
     if args.op == "backproject":
@@ -331,6 +333,8 @@ def main():
         out_h = torch.empty((cfg.n_proj, cfg.nv, cfg.nu), dtype=torch.float32).pin_memory()
         P2 = fp.Projector(*cfg.n, cfg.voxel_size, cfg.origin)
         P2.set_option(fp.OPT_INTERP, interp)
+        if cfg.cylinder:
+            P2.set_option(fp.OPT_FOV_CYLINDER, 1)
         if args.kernel:
             P2.set_option(fp.OPT_KERNEL, args.kernel)
         P2.project_host(vol_h, geom, cfg.nu, cfg.nv, out_host=out_h)          # warm-up (allocations)

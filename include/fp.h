@@ -87,7 +87,14 @@ enum {
     FP_OPT_PERMUTED_COPY = 4,
     /* 1: fp_project accumulates the number of samples sum(i_last - i_first + 1) for
      * fp_last_sample_count (default 1; one atomic per thread block). */
-    FP_OPT_COUNT_SAMPLES = 5
+    FP_OPT_COUNT_SAMPLES = 5,
+    /* 1: the caller promises that the volume is ZERO outside the cylinder about the z axis through the grid
+     * centre ((nx-1)/2, (ny-1)/2) with diameter min(nx, ny) voxels (the paper's benchmark object: "a cylindric
+     * volume within a cubic bounding box", Fig. 9).  The aligned / TMA kernels then skip
+     * the slices of a ray on which every tap lies outside that cylinder; for such a volume the result is the
+     * same sum.  The direct kernel ignores the option; fp_last_sample_count keeps counting the box samples.
+     * Default 0. */
+    FP_OPT_FOV_CYLINDER = 6
 };
 
 enum { FP_KERNEL_AUTO = 0, FP_KERNEL_DIRECT = 1, FP_KERNEL_ALIGNED = 2, FP_KERNEL_TMA = 3 };

@@ -26,6 +26,7 @@ struct fp_ctx {
     int opt_interp = FP_INTERP_LINEAR;
     int opt_permuted = 1;
     int opt_count = 1;
+    int opt_fov = 0;
     // layout stage: y-fastest copy [nz][nx][ny] for z-driven rays
     float *vol_perm = nullptr;
     const float *perm_src = nullptr;
@@ -151,6 +152,7 @@ extern "C" fp_status fp_set_option(fp_ctx *c, int key, int value)
         c->perm_valid = false;
         return FP_OK;
     case FP_OPT_COUNT_SAMPLES: c->opt_count = value != 0; return FP_OK;
+    case FP_OPT_FOV_CYLINDER: c->opt_fov = value != 0; return FP_OK;
     }
     return fail(c, FP_ERR_INVALID_ARG, "unknown option key");
 }
@@ -164,6 +166,7 @@ extern "C" fp_status fp_get_option(fp_ctx *c, int key, int *value)
     case FP_OPT_INTERP: *value = c->opt_interp; return FP_OK;
     case FP_OPT_PERMUTED_COPY: *value = c->opt_permuted; return FP_OK;
     case FP_OPT_COUNT_SAMPLES: *value = c->opt_count; return FP_OK;
+    case FP_OPT_FOV_CYLINDER: *value = c->opt_fov; return FP_OK;
     }
     return fail(c, FP_ERR_INVALID_ARG, "unknown option key");
 }
@@ -545,6 +548,7 @@ extern "C" fp_status fp_project(fp_ctx *c, const float *vol_dev, int n_proj, con
         T.nu = nu;
         T.nv = nv;
         T.n_sel = (int)ids_tm.size();
+        T.fov = c->opt_fov;
         dim3 grid((unsigned)((nu + kTmTU - 1) / kTmTU), (unsigned)((nv + kTmRows - 1) / kTmRows), (unsigned)ids_tm.size());
         s = c->opt_interp == FP_INTERP_SPLINE ? launch_tma<1>(c, T, grid, st) : launch_tma<0>(c, T, grid, st);
         if (s != FP_OK) return s;
@@ -562,6 +566,7 @@ extern "C" fp_status fp_project(fp_ctx *c, const float *vol_dev, int n_proj, con
         A.nu = nu;
         A.nv = nv;
         A.n_sel = (int)ids_al.size();
+        A.fov = c->opt_fov;
         dim3 grid((unsigned)((nu + kAlTU - 1) / kAlTU), (unsigned)((nv + kAlTV - 1) / kAlTV), (unsigned)ids_al.size());
         s = c->opt_interp == FP_INTERP_SPLINE ? launch_aligned<1>(c, A, w_al, grid, st)
                                               : launch_aligned<0>(c, A, w_al, grid, st);

@@ -36,6 +36,7 @@ struct AlignedParams {
     unsigned long long *sample_count;  // may be null
     unsigned int *err_flag;            // set to 1 if a staging window would overflow
     int nu, nv, n_sel;
+    int fov;                           // 1: the volume is zero outside the inscribed cylinder about z (FP_OPT_FOV_CYLINDER)
 };
 
 struct AlColumn {          // per detector column, constant over the slice loop
@@ -207,10 +208,16 @@ fp_aligned_kernel(const __grid_constant__ AlignedParams P)
         C.stride_s = m ? ny * nz : nz;
         C.n_s = m ? P.G.n[0] : P.G.n[1];
         int lo = 0, hi = (m ? P.G.n[1] : P.G.n[0]) - 1;
-        if (iu0 + tid < P.nu && rm != 0.0)
+        if (iu0 + tid < P.nu && rm != 0.0) {
             clip_axis(C.s_s, C.s_m, C.rt_s, C.n_s, lo, hi);
-        else
+            if (P.fov && lo <= hi) {
+                // samples whose taps (p_s +- 1) all lie outside the cylinder read zeros: skip those slices
+                const double cx = 0.5 * (P.G.n[0] - 1), cy = 0.5 * (P.G.n[1] - 1), rad = 0.5 * min(P.G.n[0], P.G.n[1]) + 1.5;
+                clip_circle(C.s_s, C.s_m, C.rt_s, m ? cy : cx, m ? cx : cy, rad, lo, hi);
+            }
+        } else {
             hi = -1;
+        }
         if (lo > hi) { lo = 0; hi = -1; }
         C.i_lo = lo;
         C.i_hi = hi;

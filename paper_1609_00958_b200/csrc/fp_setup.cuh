@@ -99,6 +99,28 @@ __device__ __forceinline__ void clip_axis(double s_t, double s_m, double rt_t, i
     hi = b < hi ? b : hi;
 }
 
+// Field-of-view clip (FP_OPT_FOV_CYLINDER; Fig. 9: "projections of a cylindric volume within a
+// cubic bounding box"): intersect [lo, hi] with the slices whose sample point (i, p_s(i)) in the (driving axis,
+// in-plane transverse axis) plane lies within radius rm of the centre (c_m, c_s).  rm already holds the margin
+// that keeps every tap of a dropped sample outside the cylinder; the quadratic is solved in fp64 and the range
+// widened by one slice on either side, so the clip is conservative.
+__device__ __forceinline__ void clip_circle(double s_s, double s_m, double rt_s, double c_m, double c_s, double rm,
+                                            int &lo, int &hi)
+{
+    const double q = s_s - s_m * rt_s - c_s;                 // p_s(i) - c_s = q + i rt_s
+    const double A = 1.0 + rt_s * rt_s, B = q * rt_s - c_m, C = c_m * c_m + q * q - rm * rm;   // A i^2 + 2 B i + C <= 0
+    const double disc = B * B - A * C;
+    if (!(disc >= 0.0)) {
+        hi = lo - 1;
+        return;
+    }
+    const double sq = sqrt(disc);
+    const int a = clamp_to_int(floor((-B - sq) / A) - 1.0, lo, hi + 1);
+    const int b = clamp_to_int(ceil((-B + sq) / A) + 1.0, lo - 1, hi);
+    lo = max(lo, a);
+    hi = min(hi, b);
+}
+
 // Transverse axes as the sampling kernels order them: (slow, fast) = (y,z), (x,z), (x,y) for
 // m = x, y, z.  The fast one is contiguous in memory for the layout the kernel reads.
 __device__ __forceinline__ int axis_slow(int m) { return m == 0 ? 1 : 0; }

@@ -42,6 +42,7 @@ struct __align__(64) TmaParams {
     unsigned long long *sample_count;  // may be null
     unsigned int *err_flag;
     int nu, nv, n_sel;
+    int fov;                           // 1: the volume is zero outside the inscribed cylinder about z (FP_OPT_FOV_CYLINDER)
 };
 
 struct TmColumn {          // per detector column and pass, all parametrised along the pass axis
@@ -120,6 +121,10 @@ __device__ __forceinline__ void tm_pass_setup(TmShared &S, const TmaParams &P, i
     if (active) {
         hi = n_m - 1;
         clip_axis(s_s, s_m, rt, n_s, lo, hi);
+        if (P.fov && lo <= hi) {
+            const double cx = 0.5 * (P.G.n[0] - 1), cy = 0.5 * (P.G.n[1] - 1), rad = 0.5 * min(P.G.n[0], P.G.n[1]) + 1.5;
+            clip_circle(s_s, s_m, rt, pass ? cy : cx, pass ? cx : cy, rad, lo, hi);
+        }
         if (lo > hi) { lo = 0; hi = -1; }
     }
     const unsigned act = __ballot_sync(0xffffffffu, active) & 0xffu;

@@ -47,6 +47,7 @@ class Config:
     nv: int
     pitch: float
     batch: Optional[int] = None      # projections per fp_project call (None = all)
+    cylinder: bool = False           # zero the volume outside the inscribed cylinder about z
 
     @property
     def seed(self) -> int:
@@ -75,9 +76,9 @@ CONFIGS = {
     # Paper-shaped workload (SURVEY.md 8(f) #4; PAPER.md:312 sec. 3.2, :283 Eq. 17): 512^3 box, 512^2 detector,
     # 10 degree full cone, 360 angles, grid matched by Eq. 17 (voxel pitch 1): S = 256 / sin 5deg, D = S / 2,
     # detector pitch (S + D) tan 5deg / 256.  Not a BASELINE.json config; the volume is the C3 phantom (the
-    # paper's cylinder data is not available) and rays are not clipped to a cylinder.
+    # paper's data is not available) set to zero outside the inscribed cylinder about z, the paper's object shape.
     "P1": Config("P1", 6, (512, 512, 512), 1.0, 40, (10.0, 160.0), "gauss", 0.01,
-                 "circular", 360, 2937.2705908915, 4405.9058863372, 512, 512, 1.5057297563),
+                 "circular", 360, 2937.2705908915, 4405.9058863372, 512, 512, 1.5057297563, cylinder=True),
 }
 
 
@@ -155,6 +156,10 @@ def make_volume(cfg: Config, device: str = "cpu"):
                 vol[x0:x1] += torch.randn(shape, generator=g, device=dev, dtype=dt) * cfg.noise_amp
             else:
                 vol[x0:x1] += (torch.rand(shape, generator=g, device=dev, dtype=dt) * 2 - 1) * cfg.noise_amp
+    if cfg.cylinder:
+        ix = torch.arange(nx, device=dev, dtype=dt).view(nx, 1, 1) - 0.5 * (nx - 1)
+        iy = torch.arange(ny, device=dev, dtype=dt).view(1, ny, 1) - 0.5 * (ny - 1)
+        vol *= ((ix * ix + iy * iy) <= (0.5 * min(nx, ny)) ** 2).to(dt)
     return vol.contiguous()
 
 

@@ -542,3 +542,36 @@ def test_aligned_class_kernels_on_degenerate_grids_and_detectors(torch, fp, orac
             worst, _, _ = compare_full(torch, fp, oracle, vol, 1.0, origin, geom, nu, nv,
                                        options=[(fp.OPT_KERNEL, opt)], what="%s %s %dx%d" % (kernel_opt, shape, nu, nv))
             assert worst < 1.0
+
+
+@pytest.mark.parametrize("kernel_opt", ["tma", "aligned"])
+def test_cylinder_field_of_view_option(torch, fp, oracle, kernel_opt):
+    """FP_OPT_FOV_CYLINDER: for a volume that is zero outside the inscribed cylinder about z the clipped slice
+    ranges give the same sums (only exact zeros are dropped; the batches start on other slices, so the fp32
+    rounding of positions and the summation order differ) and match the oracle."""
+    rng = np.random.default_rng(91)
+    opt = fp.KERNEL_TMA if kernel_opt == "tma" else fp.KERNEL_ALIGNED
+    shape, delta = (30, 26, 16), 1.0
+    origin = tuple(-(n - 1) / 2.0 for n in shape)
+    vol = rng.uniform(0.5, 1.5, size=shape).astype(np.float32)
+    ix = np.arange(shape[0])[:, None, None] - 0.5 * (shape[0] - 1)
+    iy = np.arange(shape[1])[None, :, None] - 0.5 * (shape[1] - 1)
+    vol *= ((ix * ix + iy * iy) <= (0.5 * min(shape[0], shape[1])) ** 2)
+    assert (vol == 0).mean() > 0.2
+    nu, nv = 64, 20
+    geom = np.stack([aligned_pose(th, 60.0, 120.0, nu, nv, 1.1, src_z=1.0, det_shift=(1.5, 0.0))
+                     for th in np.linspace(0.0, 2 * math.pi, 13)[:-1]])
+    volt = torch.from_numpy(vol).cuda()
+    with fp.Projector(*shape, delta, origin) as P:
+        P.set_option(fp.OPT_KERNEL, opt)
+        assert all(P.plan(g, nu, nv)[0] == opt for g in geom)
+        box = P.project(volt, geom, nu, nv).cpu().numpy()
+        P.set_option(fp.OPT_FOV_CYLINDER, 1)
+        assert P.get_option(fp.OPT_FOV_CYLINDER) == 1
+        cyl = P.project(volt, geom, nu, nv).cpu().numpy()
+        mfl = P.ray_ranges(geom, nu, nv).cpu().numpy()
+    assert np.abs(box - cyl).max() <= 1e-5 * np.abs(box).max()
+    assert np.array_equal(box == 0, cyl == 0)
+    ids = all_ids(len(geom), nv, nu)
+    ov, om, pl, mg = oracle.project_rays(vol, delta, origin, geom, ids, threads=oracle.host_cores())
+    assert assert_parity(cyl.ravel(), mfl.reshape(-1, 3), ov, om, pl, mg, float(np.abs(vol).max())) < 1.0
