@@ -15,6 +15,7 @@
 #include "fp_kernels.cuh"
 #include "fp_aligned.cuh"
 #include "fp_tma.cuh"
+#include "fp_tex.cuh"
 
 using namespace fpk;
 
@@ -27,6 +28,8 @@ struct fp_ctx {
     int opt_permuted = 1;
     int opt_count = 1;
     int opt_fov = 0;
+    int opt_tex_cols = 0;                      // columns per block of fp_tma_kernel sampled through the texture pipe (0 or 2)
+    int opt_tex_share = 0;                     // percent of a call's TMA-kernel projections that go to fp_tex_kernel instead
     // layout stage: y-fastest copy [nz][nx][ny] for z-driven rays
     float *vol_perm = nullptr;
     const float *perm_src = nullptr;
@@ -35,12 +38,23 @@ struct fp_ctx {
     ProjDesc *proj_dev = nullptr;
     int proj_cap = 0;
     unsigned long long *count_dev = nullptr;   // [0] sample count, [1] (low word) staging-window error flag
-    int *ids_dev = nullptr;                    // [3 * ids_cap]: aligned ids, direct ids, TMA ids
+    int *ids_dev = nullptr;                    // [4 * ids_cap]: aligned ids, direct ids, TMA ids, texture-kernel ids
     int ids_cap = 0;
     bool aligned_attr_set = false;
     // tensor maps of the TMA kernel: valid for one volume pointer
     CUtensorMap tmap[2][kTmWBoxes][kTmMaps];
     const float *tmap_vol = nullptr;
+    // layout stage of fp_tex_kernel: one layered 2-D array per driving axis (layer = slice), its surface (fill
+    // kernel) and two texture objects over it (point sampling for tld4, linear filtering for GJP_hwlin)
+    cudaArray_t arr[3] = {nullptr, nullptr, nullptr};
+    cudaSurfaceObject_t surf[3] = {0, 0, 0};
+    cudaTextureObject_t atex[3][2] = {{0, 0}, {0, 0}, {0, 0}};
+    const float *arr_src[3] = {nullptr, nullptr, nullptr};
+    bool arr_valid[3] = {false, false, false};
+    // second stream: fp_tex_kernel runs beside fp_tma_kernel / fp_direct_kernel on part of a call's projections
+    cudaStream_t side = nullptr;
+    cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
+    int n_sm = 0;
     cudaStream_t last_stream = nullptr;
     bool counted = false;
     int last_launches = 0;
@@ -123,6 +137,15 @@ extern "C" fp_status fp_destroy(fp_ctx *c)
     cudaFree(c->count_dev);
     cudaFree(c->ids_dev);
     cudaFree(c->hvol_dev);
+    for (int a = 0; a < 3; ++a) {
+        for (int f = 0; f < 2; ++f)
+            if (c->atex[a][f]) cudaDestroyTextureObject(c->atex[a][f]);
+        if (c->surf[a]) cudaDestroySurfaceObject(c->surf[a]);
+        if (c->arr[a]) cudaFreeArray(c->arr[a]);
+    }
+    if (c->side) cudaStreamDestroy(c->side);
+    if (c->ev_fork) cudaEventDestroy(c->ev_fork);
+    if (c->ev_join) cudaEventDestroy(c->ev_join);
     for (int k = 0; k < 2; ++k) {
         cudaFree(c->hout_dev[k]);
         if (c->hstream[k]) cudaStreamDestroy(c->hstream[k]);
@@ -139,7 +162,7 @@ extern "C" fp_status fp_set_option(fp_ctx *c, int key, int value)
     if (!c) return FP_ERR_INVALID_ARG;
     switch (key) {
     case FP_OPT_KERNEL:
-        if (value < FP_KERNEL_AUTO || value > FP_KERNEL_TMA) return fail(c, FP_ERR_INVALID_ARG, "bad kernel variant");
+        if (value < FP_KERNEL_AUTO || value > FP_KERNEL_HWLIN) return fail(c, FP_ERR_INVALID_ARG, "bad kernel variant");
         c->opt_kernel = value;
         return FP_OK;
     case FP_OPT_VOLATILE: c->opt_volatile = value != 0; return FP_OK;
@@ -153,6 +176,14 @@ extern "C" fp_status fp_set_option(fp_ctx *c, int key, int value)
         return FP_OK;
     case FP_OPT_COUNT_SAMPLES: c->opt_count = value != 0; return FP_OK;
     case FP_OPT_FOV_CYLINDER: c->opt_fov = value != 0; return FP_OK;
+    case FP_OPT_TEX_COLUMNS:
+        if (value != 0 && value != 2) return fail(c, FP_ERR_INVALID_ARG, "FP_OPT_TEX_COLUMNS must be 0 or 2");
+        c->opt_tex_cols = value;
+        return FP_OK;
+    case FP_OPT_TEX_SHARE:
+        if (value < 0 || value > 100) return fail(c, FP_ERR_INVALID_ARG, "FP_OPT_TEX_SHARE must be 0 .. 100 (percent)");
+        c->opt_tex_share = value;
+        return FP_OK;
     }
     return fail(c, FP_ERR_INVALID_ARG, "unknown option key");
 }
@@ -167,6 +198,8 @@ extern "C" fp_status fp_get_option(fp_ctx *c, int key, int *value)
     case FP_OPT_PERMUTED_COPY: *value = c->opt_permuted; return FP_OK;
     case FP_OPT_COUNT_SAMPLES: *value = c->opt_count; return FP_OK;
     case FP_OPT_FOV_CYLINDER: *value = c->opt_fov; return FP_OK;
+    case FP_OPT_TEX_SHARE: *value = c->opt_tex_share; return FP_OK;
+    case FP_OPT_TEX_COLUMNS: *value = c->opt_tex_cols; return FP_OK;
     }
     return fail(c, FP_ERR_INVALID_ARG, "unknown option key");
 }
@@ -178,19 +211,24 @@ extern "C" fp_status fp_get_option(fp_ctx *c, int key, int *value)
 // plane in two convex polygons (one per sign of r_z): clip the rectangle against the four half
 // planes of each.  Conservative (closed half planes); only decides whether the permuted copy
 // is worth building -- the kernels are correct either way.
-static bool has_z_driven(const double *g, int nu, int nv)
+static bool has_axis_driven(const double *g, int nu, int nv, int axis);
+static bool has_z_driven(const double *g, int nu, int nv) { return has_axis_driven(g, nu, nv, 2); }
+
+// The same for any axis: does some ray of the pose have `axis` as its largest direction component?
+static bool has_axis_driven(const double *g, int nu, int nv, int axis)
 {
+    const int o1 = (axis + 1) % 3, o2 = (axis + 2) % 3;
     const double c0[3] = {g[3] - g[0], g[4] - g[1], g[5] - g[2]};   // r at (0,0)
     for (int sign = -1; sign <= 1; sign += 2) {
         // polygon in (iu, iv)
         std::vector<std::pair<double, double>> poly = {
             {-0.5, -0.5}, {nu - 0.5, -0.5}, {nu - 0.5, nv - 0.5}, {-0.5, nv - 0.5}};
         for (int k = 0; k < 4 && !poly.empty(); ++k) {
-            const int ax = k >> 1;                       // x or y
-            const double sg = (k & 1) ? 1.0 : -1.0;      // sign*r_z -/+ r_ax >= 0
-            const double A = sign * c0[2] + sg * c0[ax];
-            const double B = sign * g[6 + 2] + sg * g[6 + ax];
-            const double C = sign * g[9 + 2] + sg * g[9 + ax];
+            const int ax = (k >> 1) ? o2 : o1;           // the two other axes
+            const double sg = (k & 1) ? 1.0 : -1.0;      // sign*r_axis -/+ r_ax >= 0
+            const double A = sign * c0[axis] + sg * c0[ax];
+            const double B = sign * g[6 + axis] + sg * g[6 + ax];
+            const double C = sign * g[9 + axis] + sg * g[9 + ax];
             std::vector<std::pair<double, double>> nxt;
             const size_t n = poly.size();
             for (size_t q = 0; q < n; ++q) {
@@ -238,9 +276,11 @@ static int plan_lane_v(const double *g, int nu, int nv, bool permuted)
 // 16-byte aligned volume (float4 loads along z).  The window bound is conservative: the largest
 // ray parameter |t| = |(i - s_m) / r_m| over all slices a batch can touch, times the r_z spread
 // of the rows of one block, plus the drift inside a batch, alignment and tap margins.
-static int plan_aligned(const fp_ctx *c, const float *vol, const double *g, int nu, int nv, int *tile_rows = nullptr)
+static int plan_aligned(const fp_ctx *c, const float *vol, const double *g, int nu, int nv, int *tile_rows = nullptr,
+                        int *tile_rows6 = nullptr)
 {
     if (tile_rows) *tile_rows = 1 << 30;
+    if (tile_rows6) *tile_rows6 = 1 << 30;
     for (int k = 0; k < 12; ++k)
         if (!std::isfinite(g[k])) return 0;
     if (g[8] != 0.0 || g[9] != 0.0 || g[10] != 0.0 || g[11] == 0.0) return 0;
@@ -292,19 +332,23 @@ static int plan_aligned(const fp_ctx *c, const float *vol, const double *g, int 
     if (tile_rows) {
         // volume rows one block of fp_tma_kernel needs per slice: the columns of a block that share a driving
         // axis spread over |i - s_m| (max r~_s - min r~_s) rows of the slice plane, plus the two taps
-        int rows = 0;
-        for (int iu0 = 0; iu0 < nu; iu0 += kTmTU)
-            for (int m = 0; m < 2; ++m) {
-                double lo = INFINITY, hi = -INFINITY, d = 0.0;
-                for (int iu = iu0; iu < std::min(nu, iu0 + kTmTU); ++iu)
-                    if (cols[iu].m == m) {
-                        lo = std::min(lo, cols[iu].rt);
-                        hi = std::max(hi, cols[iu].rt);
-                        d = std::max(d, cols[iu].dmax);
-                    }
-                if (lo <= hi) rows = std::max(rows, (int)std::min(d * (hi - lo), 1.0e6) + 3);
-            }
-        *tile_rows = rows;
+        // (tile_rows6: the same over the first six columns of every block, the tile columns of the <6, 2> variant)
+        for (int width = kTmTU; width >= 6; width -= 2) {
+            int rows = 0;
+            for (int iu0 = 0; iu0 < nu; iu0 += kTmTU)
+                for (int m = 0; m < 2; ++m) {
+                    double lo = INFINITY, hi = -INFINITY, d = 0.0;
+                    for (int iu = iu0; iu < std::min(nu, iu0 + width); ++iu)
+                        if (cols[iu].m == m) {
+                            lo = std::min(lo, cols[iu].rt);
+                            hi = std::max(hi, cols[iu].rt);
+                            d = std::max(d, cols[iu].dmax);
+                        }
+                    if (lo <= hi) rows = std::max(rows, (int)std::min(d * (hi - lo), 1.0e6) + 3);
+                }
+            if (width == kTmTU) *tile_rows = rows;
+            else if (tile_rows6) *tile_rows6 = rows;
+        }
     }
     return (int)std::ceil(span) + 10;
 }
@@ -319,7 +363,7 @@ static fp_status ensure_ids(fp_ctx *c, int n_proj)
         c->ids_cap = 0;
     }
     const int cap = n_proj + 64;
-    FP_CUDA(c, cudaMalloc(&c->ids_dev, sizeof(int) * 3 * (size_t)cap));
+    FP_CUDA(c, cudaMalloc(&c->ids_dev, sizeof(int) * 4 * (size_t)cap));
     c->ids_cap = cap;
     return FP_OK;
 }
@@ -328,11 +372,8 @@ template <int INTERP, int W>
 static fp_status launch_aligned_w(fp_ctx *c, const AlignedParams &A, dim3 grid, cudaStream_t st)
 {
     constexpr size_t smem = aligned_smem_bytes<W>();
-    static bool attr_set = false;      // per process and instantiation; harmless to repeat
-    if (!attr_set) {
-        FP_CUDA(c, cudaFuncSetAttribute(fp_aligned_kernel<INTERP, W>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        attr_set = true;
-    }
+    // the attribute is per device; setting it on every launch is cheap
+    FP_CUDA(c, cudaFuncSetAttribute(fp_aligned_kernel<INTERP, W>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     fp_aligned_kernel<INTERP, W><<<grid, kAlTV, smem, st>>>(A);
     FP_CUDA(c, cudaGetLastError());
     return FP_OK;
@@ -387,17 +428,95 @@ static fp_status build_tensor_maps(fp_ctx *c, const float *vol)
     return FP_OK;
 }
 
-template <int INTERP>
+template <int INTERP, int NL, int NT>
 static fp_status launch_tma(fp_ctx *c, const TmaParams &T, dim3 grid, cudaStream_t st)
 {
-    static bool attr_set = false;
-    if (!attr_set) {
-        FP_CUDA(c, cudaFuncSetAttribute(fp_tma_kernel<INTERP>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)tma_smem_bytes()));
-        attr_set = true;
-    }
-    fp_tma_kernel<INTERP><<<grid, kTmThreads, tma_smem_bytes(), st>>>(T);
+    // per device and cheap: set on every launch
+    const size_t smem = tma_smem_bytes<NL>();
+    FP_CUDA(c, cudaFuncSetAttribute(fp_tma_kernel<INTERP, NL, NT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    fp_tma_kernel<INTERP, NL, NT><<<grid, kTmThreads, smem, st>>>(T);
     FP_CUDA(c, cudaGetLastError());
     return FP_OK;
+}
+
+// Layout stage of fp_tex_kernel (sec. 2.8): the layered array of driving axis `axis`
+// (layer = slice, row = slow transverse axis, column = fast transverse axis), filled from the caller's volume
+// on `st`.  Arrays, surfaces and texture objects are created once per context.
+static fp_status ensure_layers(fp_ctx *c, const float *vol, int axis, cudaStream_t st)
+{
+    const int nx = c->G.n[0], ny = c->G.n[1], nz = c->G.n[2];
+    const int n_layer = c->G.n[axis];
+    const int n_row = axis == 0 ? ny : nx, n_col = axis == 2 ? ny : nz;
+    if (!c->arr[axis]) {
+        int dev = 0, lim[3] = {0, 0, 0};
+        FP_CUDA(c, cudaGetDevice(&dev));
+        FP_CUDA(c, cudaDeviceGetAttribute(&lim[0], cudaDevAttrMaxTexture2DLayeredWidth, dev));
+        FP_CUDA(c, cudaDeviceGetAttribute(&lim[1], cudaDevAttrMaxTexture2DLayeredHeight, dev));
+        FP_CUDA(c, cudaDeviceGetAttribute(&lim[2], cudaDevAttrMaxTexture2DLayeredLayers, dev));
+        if (n_col > lim[0] || n_row > lim[1] || n_layer > lim[2])
+            return fail(c, FP_ERR_UNSUPPORTED, "volume too large for a layered texture array on this device");
+        cudaChannelFormatDesc cd = cudaCreateChannelDesc<float>();
+        FP_CUDA(c, cudaMalloc3DArray(&c->arr[axis], &cd, make_cudaExtent((size_t)n_col, (size_t)n_row, (size_t)n_layer),
+                                     cudaArrayLayered | cudaArraySurfaceLoadStore));
+        cudaResourceDesc rd;
+        memset(&rd, 0, sizeof rd);
+        rd.resType = cudaResourceTypeArray;
+        rd.res.array.array = c->arr[axis];
+        FP_CUDA(c, cudaCreateSurfaceObject(&c->surf[axis], &rd));
+        for (int f = 0; f < 2; ++f) {
+            cudaTextureDesc td;
+            memset(&td, 0, sizeof td);
+            td.addressMode[0] = td.addressMode[1] = td.addressMode[2] = cudaAddressModeBorder;   // outside: 0 (reading #2)
+            td.filterMode = f ? cudaFilterModeLinear : cudaFilterModePoint;
+            td.readMode = cudaReadModeElementType;
+            td.normalizedCoords = 0;
+            FP_CUDA(c, cudaCreateTextureObject(&c->atex[axis][f], &rd, &td, nullptr));
+        }
+    }
+    if (axis < 2) {
+        dim3 grid((unsigned)nx, (unsigned)((ny + 7) / 8));
+        if (axis == 0) fp_fill_layers_kernel<0><<<grid, 256, 0, st>>>(vol, c->surf[0], nx, ny, nz);
+        else fp_fill_layers_kernel<1><<<grid, 256, 0, st>>>(vol, c->surf[1], nx, ny, nz);
+    } else {
+        dim3 grid((unsigned)((nz + 31) / 32), (unsigned)((ny + 31) / 32), (unsigned)nx);
+        fp_fill_layers_kernel<2><<<grid, 256, 0, st>>>(vol, c->surf[2], nx, ny, nz);
+    }
+    FP_CUDA(c, cudaGetLastError());
+    c->arr_src[axis] = vol;
+    c->arr_valid[axis] = true;
+    c->last_launches += 1;
+    return FP_OK;
+}
+
+template <int INTERP, bool HW, int U>
+static fp_status launch_tex_u(fp_ctx *c, const TexParams &T, int blocks_per_sm, cudaStream_t st)
+{
+    // beside fp_tma_kernel: four warps x 136 registers fit in what four of its 72-register blocks leave on an SM
+    const int threads = blocks_per_sm == 1 ? 96 : kTexThreads;
+    // the same shared-memory carve-out as fp_tma_kernel's blocks, or the two kernels cannot share an SM
+    if (blocks_per_sm == 1)
+        FP_CUDA(c, cudaFuncSetAttribute(fp_tex_kernel<INTERP, HW, U>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
+    int occ = 0;
+    FP_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fp_tex_kernel<INTERP, HW, U>, threads, 0));
+    const int per_sm = blocks_per_sm > 0 ? std::min(blocks_per_sm, std::max(occ, 1)) : std::max(occ, 1);
+    fp_tex_kernel<INTERP, HW, U><<<(unsigned)(c->n_sm * per_sm), threads, 0, st>>>(T);
+    FP_CUDA(c, cudaGetLastError());
+    return FP_OK;
+}
+
+// blocks_per_sm = 0: as many persistent blocks as fit (the kernel runs alone); 1: one block per SM with many
+// samples in flight per thread (beside fp_tma_kernel, in the registers that kernel leaves free)
+static fp_status launch_tex(fp_ctx *c, const TexParams &T, bool hw, int blocks_per_sm, cudaStream_t st)
+{
+    if (!c->n_sm) {
+        int dev = 0;
+        FP_CUDA(c, cudaGetDevice(&dev));
+        FP_CUDA(c, cudaDeviceGetAttribute(&c->n_sm, cudaDevAttrMultiProcessorCount, dev));
+    }
+    const bool spl = c->opt_interp == FP_INTERP_SPLINE;
+    if (hw) return launch_tex_u<0, true, 1>(c, T, 0, st);
+    if (blocks_per_sm == 1) return spl ? launch_tex_u<1, false, 16>(c, T, 1, st) : launch_tex_u<0, false, 16>(c, T, 1, st);
+    return spl ? launch_tex_u<1, false, 8>(c, T, 0, st) : launch_tex_u<0, false, 8>(c, T, 0, st);
 }
 
 static fp_status ensure_proj(fp_ctx *c, int n_proj)
@@ -491,13 +610,19 @@ extern "C" fp_status fp_project(fp_ctx *c, const float *vol_dev, int n_proj, con
     if (n_proj == 0) return FP_OK;
 
     // plan: which kernel takes which projection
-    std::vector<int> ids_al, ids_di, ids_tm;
-    int w_al = 0;
+    std::vector<int> ids_al, ids_di, ids_tm, ids_tx;
+    int w_al = 0, tile_rows_max = 0;
+    const bool all_tex = c->opt_kernel == FP_KERNEL_TEX || c->opt_kernel == FP_KERNEL_HWLIN;
     for (int p = 0; p < n_proj; ++p) {
-        int rows = 0;
-        const int w = c->opt_kernel == FP_KERNEL_DIRECT ? 0 : plan_aligned(c, vol_dev, geom + 12 * (size_t)p, nu, nv, &rows);
+        if (all_tex) {
+            ids_tx.push_back(p);
+            continue;
+        }
+        int rows = 0, rows6 = 0;
+        const int w = c->opt_kernel == FP_KERNEL_DIRECT ? 0 : plan_aligned(c, vol_dev, geom + 12 * (size_t)p, nu, nv, &rows, &rows6);
         if (w > 0 && w <= kTmW && rows <= kTmNR && c->opt_kernel != FP_KERNEL_ALIGNED) {
             ids_tm.push_back(p);                       // fits the TMA-fed kernel's tile
+            tile_rows_max = std::max(tile_rows_max, rows6);
         } else if (w > 0 && w <= kAlignedMaxW) {
             ids_al.push_back(p);
             w_al = std::max(w_al, w);
@@ -505,6 +630,15 @@ extern "C" fp_status fp_project(fp_ctx *c, const float *vol_dev, int n_proj, con
             ids_di.push_back(p);
         }
     }
+    // the texture pipe beside the shared-memory pipe: the last FP_OPT_TEX_SHARE percent of the TMA kernel's
+    // projections go to fp_tex_kernel, which runs concurrently on a second stream (AUTO only; worth the
+    // layout stage only for calls with many projections)
+    if (c->opt_kernel == FP_KERNEL_AUTO && c->opt_tex_share > 0 && ids_tm.size() >= 16) {
+        const size_t n_tx = std::min(ids_tm.size(), (ids_tm.size() * (size_t)c->opt_tex_share + 50) / 100);
+        ids_tx.assign(ids_tm.end() - (long)n_tx, ids_tm.end());
+        ids_tm.resize(ids_tm.size() - n_tx);
+    }
+    const bool hybrid = !ids_tx.empty() && !ids_tm.empty();
 
     // layout stage: only when some projection of the direct kernel has z-driven rays
     bool want_perm = false;
@@ -516,6 +650,15 @@ extern "C" fp_status fp_project(fp_ctx *c, const float *vol_dev, int n_proj, con
         if (s != FP_OK) return s;
     }
     const bool use_perm = want_perm && c->perm_valid;
+    // layout stage of the texture kernel: the layered array of every driving axis its projections have
+    for (int a = 0; a < 3 && !ids_tx.empty(); ++a) {
+        bool want = false;
+        for (size_t q = 0; q < ids_tx.size() && !want; ++q) want = has_axis_driven(geom + 12 * (size_t)ids_tx[q], nu, nv, a);
+        if (want && (!c->arr_valid[a] || c->arr_src[a] != vol_dev || c->opt_volatile)) {
+            s = ensure_layers(c, vol_dev, a, st);
+            if (s != FP_OK) return s;
+        }
+    }
 
     s = upload_geometry(c, n_proj, geom, nu, nv, use_perm, st);
     if (s != FP_OK) return s;
@@ -529,11 +672,48 @@ extern "C" fp_status fp_project(fp_ctx *c, const float *vol_dev, int n_proj, con
     if (!ids_tm.empty())
         FP_CUDA(c, cudaMemcpyAsync(c->ids_dev + 2 * c->ids_cap, ids_tm.data(), sizeof(int) * ids_tm.size(),
                                    cudaMemcpyHostToDevice, st));
+    if (!ids_tx.empty())
+        FP_CUDA(c, cudaMemcpyAsync(c->ids_dev + 3 * c->ids_cap, ids_tx.data(), sizeof(int) * ids_tx.size(),
+                                   cudaMemcpyHostToDevice, st));
 
     if (!c->count_dev) FP_CUDA(c, cudaMalloc(&c->count_dev, 2 * sizeof(unsigned long long)));
     if (!c->keep_count) FP_CUDA(c, cudaMemsetAsync(c->count_dev, 0, 2 * sizeof(unsigned long long), st));
     c->counted = c->opt_count != 0;
 
+    // the texture kernel of a hybrid call runs on the side stream, forked here and joined at the end
+    cudaStream_t st_tex = st;
+    if (hybrid) {
+        if (!c->side) FP_CUDA(c, cudaStreamCreateWithFlags(&c->side, cudaStreamNonBlocking));
+        if (!c->ev_fork) FP_CUDA(c, cudaEventCreateWithFlags(&c->ev_fork, cudaEventDisableTiming));
+        if (!c->ev_join) FP_CUDA(c, cudaEventCreateWithFlags(&c->ev_join, cudaEventDisableTiming));
+        FP_CUDA(c, cudaEventRecord(c->ev_fork, st));
+        FP_CUDA(c, cudaStreamWaitEvent(c->side, c->ev_fork, 0));
+        st_tex = c->side;
+    }
+
+    // The texture kernel goes first: its persistent grid (one block per SM in a hybrid call) is dispatched at
+    // once, and the hardware dispatches a later kernel's blocks only after every block of the earlier ones --
+    // launched second it would wait for the TMA kernel's whole grid.
+    if (!ids_tx.empty()) {
+        TexParams X;
+        X.G = c->G;
+        const int filt = c->opt_kernel == FP_KERNEL_HWLIN ? 1 : 0;
+        for (int a = 0; a < 3; ++a) X.tex[a] = (unsigned long long)c->atex[a][filt];
+        X.proj = c->proj_dev;
+        X.ids = c->ids_dev + 3 * c->ids_cap;
+        X.out = out_dev;
+        X.sample_count = c->opt_count ? c->count_dev : nullptr;
+        X.nu = nu;
+        X.nv = nv;
+        X.n_sel = (int)ids_tx.size();
+        s = launch_tex(c, X, filt != 0, hybrid ? 1 : 0, st_tex);
+        if (s != FP_OK) return s;
+        c->last_launches += 1;
+        if (hybrid) {
+            FP_CUDA(c, cudaEventRecord(c->ev_join, c->side));
+            FP_CUDA(c, cudaStreamWaitEvent(st, c->ev_join, 0));
+        }
+    }
     if (!ids_tm.empty()) {
         s = build_tensor_maps(c, vol_dev);
         if (s != FP_OK) return s;
@@ -549,8 +729,30 @@ extern "C" fp_status fp_project(fp_ctx *c, const float *vol_dev, int n_proj, con
         T.nv = nv;
         T.n_sel = (int)ids_tm.size();
         T.fov = c->opt_fov;
-        dim3 grid((unsigned)((nu + kTmTU - 1) / kTmTU), (unsigned)((nv + kTmRows - 1) / kTmRows), (unsigned)ids_tm.size());
-        s = c->opt_interp == FP_INTERP_SPLINE ? launch_tma<1>(c, T, grid, st) : launch_tma<0>(c, T, grid, st);
+        T.out_vec = ((uintptr_t)out_dev & 15) == 0 && (nu & 3) == 0;
+        // variant: beside the texture kernel 6 columns per block in 72 registers (one of its blocks fits on every SM);
+        // else with two texture columns per block when the call is large enough to pay for the layered arrays
+        const bool texcols = !hybrid && c->opt_tex_cols == 2 && tile_rows_max <= tm_nr<6>() &&
+                             ids_tm.size() >= 16;
+        if (texcols) {
+            for (int a = 0; a < 2; ++a)
+                if (!c->arr_valid[a] || c->arr_src[a] != vol_dev || c->opt_volatile) {
+                    s = ensure_layers(c, vol_dev, a, st);
+                    if (s != FP_OK) return s;
+                }
+            T.tex[0] = (unsigned long long)c->atex[0][0];
+            T.tex[1] = (unsigned long long)c->atex[1][0];
+        } else {
+            T.tex[0] = T.tex[1] = 0;
+        }
+        const int nb = hybrid ? 6 : 8;
+        dim3 grid((unsigned)((nu + nb - 1) / nb), (unsigned)((nv + kTmRows - 1) / kTmRows), (unsigned)ids_tm.size());
+        if (texcols)
+            s = c->opt_interp == FP_INTERP_SPLINE ? launch_tma<1, 6, 2>(c, T, grid, st) : launch_tma<0, 6, 2>(c, T, grid, st);
+        else if (nb == 6)
+            s = c->opt_interp == FP_INTERP_SPLINE ? launch_tma<1, 6, 0>(c, T, grid, st) : launch_tma<0, 6, 0>(c, T, grid, st);
+        else
+            s = c->opt_interp == FP_INTERP_SPLINE ? launch_tma<1, 8, 0>(c, T, grid, st) : launch_tma<0, 8, 0>(c, T, grid, st);
         if (s != FP_OK) return s;
         c->last_launches += 1;
     }
