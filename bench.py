@@ -241,8 +241,7 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--kernel", type=int, default=0, help="FP_OPT_KERNEL value (0 = auto)")
-    ap.add_argument("--tex-share", type=int, default=-1, help="FP_OPT_TEX_SHARE percent (-1 = library default)")
-    ap.add_argument("--tex-cols", type=int, default=-1, help="FP_OPT_TEX_COLUMNS (-1 = library default)")
+    ap.add_argument("--group", type=int, default=-1)
     ap.add_argument("--op", default="project", choices=["project", "backproject"],
                     help="project: the headline forward projector; backproject: its exact transpose (SURVEY 8(f) #2)")
     ap.add_argument("--interp", default="linear", choices=["linear", "spline"],
@@ -276,12 +275,10 @@ def main():
     P = fp.Projector(*cfg.n, cfg.voxel_size, cfg.origin)
     if args.kernel:
         P.set_option(fp.OPT_KERNEL, args.kernel)
-    if args.tex_share >= 0:
-        P.set_option(fp.OPT_TEX_SHARE, args.tex_share)
-    if args.tex_cols >= 0:
-        P.set_option(fp.OPT_TEX_COLUMNS, args.tex_cols)
     interp = fp.INTERP_SPLINE if args.interp == "spline" else fp.INTERP_LINEAR
     P.set_option(fp.OPT_INTERP, interp)
+    if args.group >= 0:
+        P.set_option(100, args.group)
     if cfg.cylinder:
         P.set_option(fp.OPT_FOV_CYLINDER, 1)       # the volume is zero outside the inscribed cylinder
     stream = torch.cuda.current_stream()
@@ -344,8 +341,6 @@ def main():
             P2.set_option(fp.OPT_FOV_CYLINDER, 1)
         if args.kernel:
             P2.set_option(fp.OPT_KERNEL, args.kernel)
-        if args.tex_share >= 0:
-            P2.set_option(fp.OPT_TEX_SHARE, args.tex_share)
         P2.project_host(vol_h, geom, cfg.nu, cfg.nv, out_host=out_h)          # warm-up (allocations)
         n_e2e = max(1, min(args.steps, 3))
         barrier()

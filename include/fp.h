@@ -101,18 +101,7 @@ enum {
      * the slices of a ray on which every tap lies outside that cylinder; for such a volume the result is the
      * same sum.  The direct kernel ignores the option; fp_last_sample_count keeps counting the box samples.
      * Default 0. */
-    FP_OPT_FOV_CYLINDER = 6,
-    /* FP_KERNEL_AUTO only: percent (0 .. 100, default 0) of the projections of a call planned for FP_KERNEL_TMA
-     * that are sampled by FP_KERNEL_TEX instead, CONCURRENTLY on a second stream of the library (joined into
-     * `stream` before fp_project returns control of it): the texture pipe works beside the shared-memory pipe
-     * that bounds the TMA kernel.  Applies to calls with at least 16 such projections; costs the layout stage
-     * of FP_KERNEL_TEX (one volume-sized layered array per driving axis in use). */
-    FP_OPT_TEX_SHARE = 7,
-    /* Detector columns (0 or 2, default 0) of every 8-column block of FP_KERNEL_TMA that its threads sample
-     * through the texture pipe (one tld4 per sample from the layered arrays of FP_KERNEL_TEX's layout stage,
-     * explicit fp32 weights) beside the six columns they sample from the shared-memory tile.  Used for calls
-     * with at least 16 projections of that kernel (the layout stage costs two volume copies per call). */
-    FP_OPT_TEX_COLUMNS = 8
+    FP_OPT_FOV_CYLINDER = 6
 };
 
 enum { FP_KERNEL_AUTO = 0, FP_KERNEL_DIRECT = 1, FP_KERNEL_ALIGNED = 2, FP_KERNEL_TMA = 3, FP_KERNEL_TEX = 4, FP_KERNEL_HWLIN = 5 };

@@ -28,8 +28,7 @@ struct fp_ctx {
     int opt_permuted = 1;
     int opt_count = 1;
     int opt_fov = 0;
-    int opt_tex_cols = 0;                      // columns per block of fp_tma_kernel sampled through the texture pipe (0 or 2)
-    int opt_tex_share = 0;                     // percent of a call's TMA-kernel projections that go to fp_tex_kernel instead
+    int opt_group = 4;                         // projections per launch-order group of fp_tma_kernel
     // layout stage: y-fastest copy [nz][nx][ny] for z-driven rays
     float *vol_perm = nullptr;
     const float *perm_src = nullptr;
@@ -51,9 +50,6 @@ struct fp_ctx {
     cudaTextureObject_t atex[3][2] = {{0, 0}, {0, 0}, {0, 0}};
     const float *arr_src[3] = {nullptr, nullptr, nullptr};
     bool arr_valid[3] = {false, false, false};
-    // second stream: fp_tex_kernel runs beside fp_tma_kernel / fp_direct_kernel on part of a call's projections
-    cudaStream_t side = nullptr;
-    cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
     int n_sm = 0;
     cudaStream_t last_stream = nullptr;
     bool counted = false;
@@ -143,9 +139,6 @@ extern "C" fp_status fp_destroy(fp_ctx *c)
         if (c->surf[a]) cudaDestroySurfaceObject(c->surf[a]);
         if (c->arr[a]) cudaFreeArray(c->arr[a]);
     }
-    if (c->side) cudaStreamDestroy(c->side);
-    if (c->ev_fork) cudaEventDestroy(c->ev_fork);
-    if (c->ev_join) cudaEventDestroy(c->ev_join);
     for (int k = 0; k < 2; ++k) {
         cudaFree(c->hout_dev[k]);
         if (c->hstream[k]) cudaStreamDestroy(c->hstream[k]);
@@ -176,14 +169,7 @@ extern "C" fp_status fp_set_option(fp_ctx *c, int key, int value)
         return FP_OK;
     case FP_OPT_COUNT_SAMPLES: c->opt_count = value != 0; return FP_OK;
     case FP_OPT_FOV_CYLINDER: c->opt_fov = value != 0; return FP_OK;
-    case FP_OPT_TEX_COLUMNS:
-        if (value != 0 && value != 2) return fail(c, FP_ERR_INVALID_ARG, "FP_OPT_TEX_COLUMNS must be 0 or 2");
-        c->opt_tex_cols = value;
-        return FP_OK;
-    case FP_OPT_TEX_SHARE:
-        if (value < 0 || value > 100) return fail(c, FP_ERR_INVALID_ARG, "FP_OPT_TEX_SHARE must be 0 .. 100 (percent)");
-        c->opt_tex_share = value;
-        return FP_OK;
+    case 100: c->opt_group = value; return FP_OK;   // DEV
     }
     return fail(c, FP_ERR_INVALID_ARG, "unknown option key");
 }
@@ -198,8 +184,6 @@ extern "C" fp_status fp_get_option(fp_ctx *c, int key, int *value)
     case FP_OPT_PERMUTED_COPY: *value = c->opt_permuted; return FP_OK;
     case FP_OPT_COUNT_SAMPLES: *value = c->opt_count; return FP_OK;
     case FP_OPT_FOV_CYLINDER: *value = c->opt_fov; return FP_OK;
-    case FP_OPT_TEX_SHARE: *value = c->opt_tex_share; return FP_OK;
-    case FP_OPT_TEX_COLUMNS: *value = c->opt_tex_cols; return FP_OK;
     }
     return fail(c, FP_ERR_INVALID_ARG, "unknown option key");
 }
@@ -276,11 +260,9 @@ static int plan_lane_v(const double *g, int nu, int nv, bool permuted)
 // 16-byte aligned volume (float4 loads along z).  The window bound is conservative: the largest
 // ray parameter |t| = |(i - s_m) / r_m| over all slices a batch can touch, times the r_z spread
 // of the rows of one block, plus the drift inside a batch, alignment and tap margins.
-static int plan_aligned(const fp_ctx *c, const float *vol, const double *g, int nu, int nv, int *tile_rows = nullptr,
-                        int *tile_rows6 = nullptr)
+static int plan_aligned(const fp_ctx *c, const float *vol, const double *g, int nu, int nv, int *tile_rows = nullptr)
 {
     if (tile_rows) *tile_rows = 1 << 30;
-    if (tile_rows6) *tile_rows6 = 1 << 30;
     for (int k = 0; k < 12; ++k)
         if (!std::isfinite(g[k])) return 0;
     if (g[8] != 0.0 || g[9] != 0.0 || g[10] != 0.0 || g[11] == 0.0) return 0;
@@ -332,23 +314,19 @@ static int plan_aligned(const fp_ctx *c, const float *vol, const double *g, int 
     if (tile_rows) {
         // volume rows one block of fp_tma_kernel needs per slice: the columns of a block that share a driving
         // axis spread over |i - s_m| (max r~_s - min r~_s) rows of the slice plane, plus the two taps
-        // (tile_rows6: the same over the first six columns of every block, the tile columns of the <6, 2> variant)
-        for (int width = kTmTU; width >= 6; width -= 2) {
-            int rows = 0;
-            for (int iu0 = 0; iu0 < nu; iu0 += kTmTU)
-                for (int m = 0; m < 2; ++m) {
-                    double lo = INFINITY, hi = -INFINITY, d = 0.0;
-                    for (int iu = iu0; iu < std::min(nu, iu0 + width); ++iu)
-                        if (cols[iu].m == m) {
-                            lo = std::min(lo, cols[iu].rt);
-                            hi = std::max(hi, cols[iu].rt);
-                            d = std::max(d, cols[iu].dmax);
-                        }
-                    if (lo <= hi) rows = std::max(rows, (int)std::min(d * (hi - lo), 1.0e6) + 3);
-                }
-            if (width == kTmTU) *tile_rows = rows;
-            else if (tile_rows6) *tile_rows6 = rows;
-        }
+        int rows = 0;
+        for (int iu0 = 0; iu0 < nu; iu0 += kTmTU)
+            for (int m = 0; m < 2; ++m) {
+                double lo = INFINITY, hi = -INFINITY, d = 0.0;
+                for (int iu = iu0; iu < std::min(nu, iu0 + kTmTU); ++iu)
+                    if (cols[iu].m == m) {
+                        lo = std::min(lo, cols[iu].rt);
+                        hi = std::max(hi, cols[iu].rt);
+                        d = std::max(d, cols[iu].dmax);
+                    }
+                if (lo <= hi) rows = std::max(rows, (int)std::min(d * (hi - lo), 1.0e6) + 3);
+            }
+        *tile_rows = rows;
     }
     return (int)std::ceil(span) + 10;
 }
@@ -428,16 +406,19 @@ static fp_status build_tensor_maps(fp_ctx *c, const float *vol)
     return FP_OK;
 }
 
-template <int INTERP, int NL, int NT>
+template <int INTERP>
 static fp_status launch_tma(fp_ctx *c, const TmaParams &T, dim3 grid, cudaStream_t st)
 {
     // per device and cheap: set on every launch
-    const size_t smem = tma_smem_bytes<NL>();
-    FP_CUDA(c, cudaFuncSetAttribute(fp_tma_kernel<INTERP, NL, NT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    fp_tma_kernel<INTERP, NL, NT><<<grid, kTmThreads, smem, st>>>(T);
+    const size_t smem = tma_smem_bytes();
+    FP_CUDA(c, cudaFuncSetAttribute(fp_tma_kernel<INTERP>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    fp_tma_kernel<INTERP><<<grid, kTmThreads, smem, st>>>(T);
     FP_CUDA(c, cudaGetLastError());
     return FP_OK;
 }
+
+// Does a pose with this z window and these volume rows per slice fit fp_tma_kernel's tiles?
+static bool fits_tma(int window, int rows) { return window > 0 && window <= kTmW && rows <= kTmNR; }
 
 // Layout stage of fp_tex_kernel (sec. 2.8): the layered array of driving axis `axis`
 // (layer = slice, row = slow transverse axis, column = fast transverse axis), filled from the caller's volume
@@ -488,25 +469,18 @@ static fp_status ensure_layers(fp_ctx *c, const float *vol, int axis, cudaStream
     return FP_OK;
 }
 
+// fp_tex_kernel: a persistent grid of as many blocks as fit.
 template <int INTERP, bool HW, int U>
-static fp_status launch_tex_u(fp_ctx *c, const TexParams &T, int blocks_per_sm, cudaStream_t st)
+static fp_status launch_tex_u(fp_ctx *c, const TexParams &T, cudaStream_t st)
 {
-    // beside fp_tma_kernel: four warps x 136 registers fit in what four of its 72-register blocks leave on an SM
-    const int threads = blocks_per_sm == 1 ? 96 : kTexThreads;
-    // the same shared-memory carve-out as fp_tma_kernel's blocks, or the two kernels cannot share an SM
-    if (blocks_per_sm == 1)
-        FP_CUDA(c, cudaFuncSetAttribute(fp_tex_kernel<INTERP, HW, U>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
     int occ = 0;
-    FP_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fp_tex_kernel<INTERP, HW, U>, threads, 0));
-    const int per_sm = blocks_per_sm > 0 ? std::min(blocks_per_sm, std::max(occ, 1)) : std::max(occ, 1);
-    fp_tex_kernel<INTERP, HW, U><<<(unsigned)(c->n_sm * per_sm), threads, 0, st>>>(T);
+    FP_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fp_tex_kernel<INTERP, HW, U>, kTexThreads, 0));
+    fp_tex_kernel<INTERP, HW, U><<<(unsigned)(c->n_sm * std::max(occ, 1)), kTexThreads, 0, st>>>(T);
     FP_CUDA(c, cudaGetLastError());
     return FP_OK;
 }
 
-// blocks_per_sm = 0: as many persistent blocks as fit (the kernel runs alone); 1: one block per SM with many
-// samples in flight per thread (beside fp_tma_kernel, in the registers that kernel leaves free)
-static fp_status launch_tex(fp_ctx *c, const TexParams &T, bool hw, int blocks_per_sm, cudaStream_t st)
+static fp_status launch_tex(fp_ctx *c, const TexParams &T, bool hw, cudaStream_t st)
 {
     if (!c->n_sm) {
         int dev = 0;
@@ -514,9 +488,8 @@ static fp_status launch_tex(fp_ctx *c, const TexParams &T, bool hw, int blocks_p
         FP_CUDA(c, cudaDeviceGetAttribute(&c->n_sm, cudaDevAttrMultiProcessorCount, dev));
     }
     const bool spl = c->opt_interp == FP_INTERP_SPLINE;
-    if (hw) return launch_tex_u<0, true, 1>(c, T, 0, st);
-    if (blocks_per_sm == 1) return spl ? launch_tex_u<1, false, 16>(c, T, 1, st) : launch_tex_u<0, false, 16>(c, T, 1, st);
-    return spl ? launch_tex_u<1, false, 8>(c, T, 0, st) : launch_tex_u<0, false, 8>(c, T, 0, st);
+    if (hw) return launch_tex_u<0, true, 1>(c, T, st);
+    return spl ? launch_tex_u<1, false, 8>(c, T, st) : launch_tex_u<0, false, 8>(c, T, st);
 }
 
 static fp_status ensure_proj(fp_ctx *c, int n_proj)
@@ -611,18 +584,17 @@ extern "C" fp_status fp_project(fp_ctx *c, const float *vol_dev, int n_proj, con
 
     // plan: which kernel takes which projection
     std::vector<int> ids_al, ids_di, ids_tm, ids_tx;
-    int w_al = 0, tile_rows_max = 0;
+    int w_al = 0;
     const bool all_tex = c->opt_kernel == FP_KERNEL_TEX || c->opt_kernel == FP_KERNEL_HWLIN;
     for (int p = 0; p < n_proj; ++p) {
         if (all_tex) {
             ids_tx.push_back(p);
             continue;
         }
-        int rows = 0, rows6 = 0;
-        const int w = c->opt_kernel == FP_KERNEL_DIRECT ? 0 : plan_aligned(c, vol_dev, geom + 12 * (size_t)p, nu, nv, &rows, &rows6);
-        if (w > 0 && w <= kTmW && rows <= kTmNR && c->opt_kernel != FP_KERNEL_ALIGNED) {
+        int rows = 0;
+        const int w = c->opt_kernel == FP_KERNEL_DIRECT ? 0 : plan_aligned(c, vol_dev, geom + 12 * (size_t)p, nu, nv, &rows);
+        if (fits_tma(w, rows) && c->opt_kernel != FP_KERNEL_ALIGNED) {
             ids_tm.push_back(p);                       // fits the TMA-fed kernel's tile
-            tile_rows_max = std::max(tile_rows_max, rows6);
         } else if (w > 0 && w <= kAlignedMaxW) {
             ids_al.push_back(p);
             w_al = std::max(w_al, w);
@@ -630,16 +602,6 @@ extern "C" fp_status fp_project(fp_ctx *c, const float *vol_dev, int n_proj, con
             ids_di.push_back(p);
         }
     }
-    // the texture pipe beside the shared-memory pipe: the last FP_OPT_TEX_SHARE percent of the TMA kernel's
-    // projections go to fp_tex_kernel, which runs concurrently on a second stream (AUTO only; worth the
-    // layout stage only for calls with many projections)
-    if (c->opt_kernel == FP_KERNEL_AUTO && c->opt_tex_share > 0 && ids_tm.size() >= 16) {
-        const size_t n_tx = std::min(ids_tm.size(), (ids_tm.size() * (size_t)c->opt_tex_share + 50) / 100);
-        ids_tx.assign(ids_tm.end() - (long)n_tx, ids_tm.end());
-        ids_tm.resize(ids_tm.size() - n_tx);
-    }
-    const bool hybrid = !ids_tx.empty() && !ids_tm.empty();
-
     // layout stage: only when some projection of the direct kernel has z-driven rays
     bool want_perm = false;
     if (c->opt_permuted)
@@ -680,20 +642,6 @@ extern "C" fp_status fp_project(fp_ctx *c, const float *vol_dev, int n_proj, con
     if (!c->keep_count) FP_CUDA(c, cudaMemsetAsync(c->count_dev, 0, 2 * sizeof(unsigned long long), st));
     c->counted = c->opt_count != 0;
 
-    // the texture kernel of a hybrid call runs on the side stream, forked here and joined at the end
-    cudaStream_t st_tex = st;
-    if (hybrid) {
-        if (!c->side) FP_CUDA(c, cudaStreamCreateWithFlags(&c->side, cudaStreamNonBlocking));
-        if (!c->ev_fork) FP_CUDA(c, cudaEventCreateWithFlags(&c->ev_fork, cudaEventDisableTiming));
-        if (!c->ev_join) FP_CUDA(c, cudaEventCreateWithFlags(&c->ev_join, cudaEventDisableTiming));
-        FP_CUDA(c, cudaEventRecord(c->ev_fork, st));
-        FP_CUDA(c, cudaStreamWaitEvent(c->side, c->ev_fork, 0));
-        st_tex = c->side;
-    }
-
-    // The texture kernel goes first: its persistent grid (one block per SM in a hybrid call) is dispatched at
-    // once, and the hardware dispatches a later kernel's blocks only after every block of the earlier ones --
-    // launched second it would wait for the TMA kernel's whole grid.
     if (!ids_tx.empty()) {
         TexParams X;
         X.G = c->G;
@@ -706,13 +654,9 @@ extern "C" fp_status fp_project(fp_ctx *c, const float *vol_dev, int n_proj, con
         X.nu = nu;
         X.nv = nv;
         X.n_sel = (int)ids_tx.size();
-        s = launch_tex(c, X, filt != 0, hybrid ? 1 : 0, st_tex);
+        s = launch_tex(c, X, filt != 0, st);
         if (s != FP_OK) return s;
         c->last_launches += 1;
-        if (hybrid) {
-            FP_CUDA(c, cudaEventRecord(c->ev_join, c->side));
-            FP_CUDA(c, cudaStreamWaitEvent(st, c->ev_join, 0));
-        }
     }
     if (!ids_tm.empty()) {
         s = build_tensor_maps(c, vol_dev);
@@ -730,29 +674,11 @@ extern "C" fp_status fp_project(fp_ctx *c, const float *vol_dev, int n_proj, con
         T.n_sel = (int)ids_tm.size();
         T.fov = c->opt_fov;
         T.out_vec = ((uintptr_t)out_dev & 15) == 0 && (nu & 3) == 0;
-        // variant: beside the texture kernel 6 columns per block in 72 registers (one of its blocks fits on every SM);
-        // else with two texture columns per block when the call is large enough to pay for the layered arrays
-        const bool texcols = !hybrid && c->opt_tex_cols == 2 && tile_rows_max <= tm_nr<6>() &&
-                             ids_tm.size() >= 16;
-        if (texcols) {
-            for (int a = 0; a < 2; ++a)
-                if (!c->arr_valid[a] || c->arr_src[a] != vol_dev || c->opt_volatile) {
-                    s = ensure_layers(c, vol_dev, a, st);
-                    if (s != FP_OK) return s;
-                }
-            T.tex[0] = (unsigned long long)c->atex[0][0];
-            T.tex[1] = (unsigned long long)c->atex[1][0];
-        } else {
-            T.tex[0] = T.tex[1] = 0;
-        }
-        const int nb = hybrid ? 6 : 8;
-        dim3 grid((unsigned)((nu + nb - 1) / nb), (unsigned)((nv + kTmRows - 1) / kTmRows), (unsigned)ids_tm.size());
-        if (texcols)
-            s = c->opt_interp == FP_INTERP_SPLINE ? launch_tma<1, 6, 2>(c, T, grid, st) : launch_tma<0, 6, 2>(c, T, grid, st);
-        else if (nb == 6)
-            s = c->opt_interp == FP_INTERP_SPLINE ? launch_tma<1, 6, 0>(c, T, grid, st) : launch_tma<0, 6, 0>(c, T, grid, st);
-        else
-            s = c->opt_interp == FP_INTERP_SPLINE ? launch_tma<1, 8, 0>(c, T, grid, st) : launch_tma<0, 8, 0>(c, T, grid, st);
+        // groups of neighbouring poses share their volume rows through L2 (fp_tma.cuh)
+        T.group = std::max(1, std::min(c->opt_group, (int)ids_tm.size()));
+        dim3 grid((unsigned)((nu + kTmTU - 1) / kTmTU * T.group), (unsigned)((nv + kTmRows - 1) / kTmRows),
+                  (unsigned)((ids_tm.size() + T.group - 1) / T.group));
+        s = c->opt_interp == FP_INTERP_SPLINE ? launch_tma<1>(c, T, grid, st) : launch_tma<0>(c, T, grid, st);
         if (s != FP_OK) return s;
         c->last_launches += 1;
     }
@@ -871,7 +797,7 @@ extern "C" fp_status fp_plan(fp_ctx *c, const double *geom, int nu, int nv, int 
     const int w = c->opt_kernel == FP_KERNEL_DIRECT ? 0 : plan_aligned(c, nullptr, geom, nu, nv, &rows);
     const bool al = w > 0 && w <= kAlignedMaxW;
     *kernel = al ? FP_KERNEL_ALIGNED : FP_KERNEL_DIRECT;
-    if (al && c->opt_kernel != FP_KERNEL_ALIGNED && w <= kTmW && rows <= kTmNR) *kernel = FP_KERNEL_TMA;
+    if (al && c->opt_kernel != FP_KERNEL_ALIGNED && fits_tma(w, rows)) *kernel = FP_KERNEL_TMA;
     *window = al ? w : 0;
     *z_driven = has_z_driven(geom, nu, nv) ? 1 : 0;
     return FP_OK;

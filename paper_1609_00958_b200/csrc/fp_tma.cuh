@@ -12,14 +12,10 @@
 // sample from the tile and apply the product weights of Eq. 11 (:142); each thread carries two
 // detector rows as one packed fp32x2 value.  No staging pass, no block-wide barrier in the loop.
 //
-// NL = detector columns per block sampled from the tile, NT = further columns of the block (0 or 2) that every
-// consumer thread samples through the TEXTURE pipe instead: one tld4 per sample from the layered array of the
-// pass's driving axis (fp_tex.cuh: same four taps, explicit fp32 weights), issued before the thread's tile
-// columns of the slice and used after them.  The shared-memory data pipe (LSU) is the unit this kernel
-// saturates (83 % of its wavefront peak with NT = 0); the texture pipe runs beside it (measured: a tld4 costs
-// 15.5 clk per warp whether or not the LSU is busy), so those samples come almost for free.  <8, 0>: 96
-// registers, four blocks per SM.  <6, 2>: three blocks per SM (the tld4 results in flight need the registers).
-// <6, 0>: 72 registers, five blocks per SM (beside fp_tex_kernel in a FP_OPT_TEX_SHARE call).
+// Projections are processed in groups of `group` (TmaParams): the blocks of the same detector tile of
+// the group's projections are neighbours in launch order, so they start together and sweep the volume
+// in step -- neighbouring orbit poses cut nearly the same volume rows on every slice, and whichever
+// block comes second finds them in L2.  This takes the DRAM traffic below one volume pass per projection.
 #pragma once
 #include <cstdint>
 #include <cuda.h>
@@ -27,11 +23,10 @@
 #include "fp_setup.cuh"
 #include "fp_kernels.cuh"
 #include "fp_aligned.cuh"
-#include "fp_tex.cuh"
 
 namespace fpk {
 
-constexpr int kTmTU = 8;                 // column slots per block (NL <= 8 of them carry a detector column)
+constexpr int kTmTU = 8;                 // detector columns per block
 constexpr int kTmSB = 4;                 // slices per batch = pipeline stages
 constexpr int kTmRows = 256;             // detector rows per block, two per consumer thread
 constexpr int kTmConsumers = kTmRows / 2;
@@ -39,11 +34,10 @@ constexpr int kTmThreads = kTmConsumers + 32;
 constexpr int kTmW = 256;                // largest z window (voxels) = largest inner TMA box size
 constexpr int kTmWBoxes = 4;             // inner box sizes 160, 192, 224, 256: the tile's row pitch follows the box
 constexpr int kTmWMin = 160, kTmWStep = 32;
-constexpr int kTmNR = 12;                // volume rows per tile of the 8-column variant (largest box); two zero rows follow
-// NL = 6: 10 rows per tile, 42 KB of shared memory per block, five blocks per SM
-template <int NL> __host__ __device__ constexpr int tm_nr() { return NL == 8 ? kTmNR : 10; }
-template <int NL> __host__ __device__ constexpr int tm_stage_floats() { return tm_nr<NL>() * kTmW; }
-constexpr int kTmMaps = 5;                // tensor maps per pass: boxes of 4, 6, 8, 10, 12 rows
+constexpr int kTmNR = 12;                // most volume rows per tile (largest box)
+constexpr int kTmMaps = 5;               // tensor maps per pass: boxes of 4, 6, 8, 10, 12 rows
+constexpr int kTmStageFloats = kTmNR * kTmW;
+constexpr unsigned kTmTileBytes = kTmSB * kTmStageFloats * 4u;   // 48 KB of tiles; two zero rows follow
 
 struct __align__(64) TmaParams {
     CUtensorMap map[2][kTmWBoxes][kTmMaps];   // [pass = driving axis x / y][box width][box of 4, 6, 8, 10 or 12 rows]
@@ -56,7 +50,7 @@ struct __align__(64) TmaParams {
     int nu, nv, n_sel;
     int fov;                           // 1: the volume is zero outside the inscribed cylinder about z (FP_OPT_FOV_CYLINDER)
     int out_vec;                       // 1: out is 16-byte aligned and nu % 4 == 0 (vector stores allowed)
-    unsigned long long tex[2];         // NT > 0: texture objects (point sampling) of the layered arrays of axes x and y
+    int group;                         // projections whose blocks are interleaved in launch order (>= 1)
 };
 
 struct TmColumn {          // per detector column and pass, all parametrised along the pass axis
@@ -67,16 +61,14 @@ struct TmColumn {          // per detector column and pass, all parametrised alo
 
 struct __align__(16) TmShared {
     unsigned long long full[kTmSB], empty[kTmSB];      // mbarriers
-    uint2 stage_col[kTmSB][kTmTU];     // per (stage, column): byte offset of its lower row in the tile, weight bits
-    float4 stage_tex[kTmSB][2];        // NT > 0, per (stage, texture column): row + 1 (or < 0: no sample), weight, t, z of the middle row - anchor
-    int2 stage_ti[kTmSB];              // NT > 0, per stage: slice index (= layer), float bits of the integer z anchor + 1
+    uint2 stage_col[kTmSB][kTmTU];     // per (stage, column): byte offset of its lower row in the tiles, weight bits
     double t0[2][kTmTU];               // per (batch parity, column): (i0 - s_m) / r_m
     double off[2];                     // per batch parity: s_z - z0
     unsigned pitch[2];                 // per batch parity: byte pitch of the tile rows (= box width * 4)
     TmColumn col[kTmTU];
     double s[3];                       // source, grid units
     double rxy[kTmTU][2];              // r_x, r_y per column
-    double rho_first, rho_last, rho_mid;
+    double rho_first, rho_last;
     double s_m, s_s;                   // per pass
     int n_s, n_m, i_begin, dir, n_batches, any;
 };
@@ -95,25 +87,26 @@ __device__ __forceinline__ void tm_mbar_arrive_tx(unsigned long long *bar, unsig
 {
     asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(tm_smem(bar)), "r"(bytes) : "memory");
 }
+// The suspend-time hint lets the warp sleep in hardware until the phase completes instead of spinning
+// through issue slots that the other warps of the scheduler need.
 __device__ __forceinline__ void tm_mbar_wait(unsigned long long *bar, unsigned parity)
 {
     asm volatile(
         "{\n"
         ".reg .pred p;\n"
         "WAIT_%=:\n"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1, %2;\n"
         "@p bra DONE_%=;\n"
         "bra WAIT_%=;\n"
         "DONE_%=:\n"
         "}\n" ::"r"(tm_smem(bar)),
-        "r"(parity)
+        "r"(parity), "r"(0x989680u)
         : "memory");
 }
-__device__ __forceinline__ void tm_load_3d(const CUtensorMap *map, void *dst, unsigned long long *bar, int c0, int c1, int c2)
+__device__ __forceinline__ void tm_load_3d(const CUtensorMap *map, unsigned dst, unsigned long long *bar, int c0, int c1, int c2)
 {
     asm volatile(
-        "cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5}], [%2];" ::"r"(
-            tm_smem(dst)),
+        "cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5}], [%2];" ::"r"(dst),
         "l"(map), "r"(tm_smem(bar)), "r"(c0), "r"(c1), "r"(c2)
         : "memory");
 }
@@ -123,13 +116,12 @@ __device__ __forceinline__ void tm_load_3d(const CUtensorMap *map, void *dst, un
 // past the detector edge) gets an empty slice range -- it reads the tile's zero rows -- and
 // borrows r_m from the nearest column of the pass so that its z positions stay inside the window.
 // Executed by the producer warp.
-template <int NL, int NT>
 __device__ __forceinline__ void tm_pass_setup(TmShared &S, const TmaParams &P, int pass, int iu0, int lane)
 {
     const int c = lane & (kTmTU - 1);
     const double rm = S.rxy[c][pass], rs = S.rxy[c][1 - pass];
     const int true_m = fabs(S.rxy[c][1]) > fabs(S.rxy[c][0]) ? 1 : 0;        // Eq. 2 (z excluded by the host plan)
-    const bool active = (c < NL + NT) && (true_m == pass) && (iu0 + c < P.nu) && (rm != 0.0);
+    const bool active = (true_m == pass) && (iu0 + c < P.nu) && (rm != 0.0);
     const double s_m = S.s[pass], s_s = S.s[1 - pass];
     const int n_m = P.G.n[pass], n_s = P.G.n[1 - pass];
     double inv = active ? 1.0 / rm : 0.0;
@@ -159,8 +151,7 @@ __device__ __forceinline__ void tm_pass_setup(TmShared &S, const TmaParams &P, i
     const int glo = __reduce_min_sync(0xffffffffu, has ? lo : 0x7fffffff);
     const int ghi = __reduce_max_sync(0xffffffffu, has ? hi : -1);
     // spread of the slow-axis positions over the pass's columns, in rows, at either end of the slice range
-    // (tile columns only: the texture columns need no tile rows)
-    double rt_min = (has && c < NL) ? rt : 1.0e300, rt_max = (has && c < NL) ? rt : -1.0e300;
+    double rt_min = has ? rt : 1.0e300, rt_max = has ? rt : -1.0e300;
 #pragma unroll
     for (int k = 1; k < kTmTU; k <<= 1) {
         rt_min = fmin(rt_min, __shfl_xor_sync(0xffffffffu, rt_min, k));
@@ -186,41 +177,39 @@ __device__ __forceinline__ void tm_pass_setup(TmShared &S, const TmaParams &P, i
         S.n_m = n_m;
         double spread = 0.0;
         if (any) spread = fmax(fabs((double)glo - s_m), fabs((double)(ghi + kTmSB) - s_m)) * (rt_max - rt_min);
-        if ((int)fmin(spread, 1.0e6) + 3 > tm_nr<NL>()) atomicOr(P.err_flag, 2u);
+        if ((int)fmin(spread, 1.0e6) + 3 > kTmNR) atomicOr(P.err_flag, 2u);
     }
 }
 
 // Producer warp, one batch: lane = (slice s of the batch) * 8 + column c.  Plans the four slices in
 // fp64, then per slice waits until the consumers have released the stage, publishes the per-column
-// tile row / weight and launches the TMA copy of the slice's rows x window tile.  Only the first NL
-// columns of the block are sampled from the tile.
-template <int INTERP, int NL, int NT>
-__device__ __forceinline__ void tm_produce_batch(TmShared &S, const TmaParams &P, float *tiles, int pass, int b,
+// tile row / weight and launches the TMA copy of the slice's rows x window tile.
+template <int INTERP>
+__device__ __forceinline__ void tm_produce_batch(TmShared &S, const TmaParams &P, unsigned tiles_smem, int pass, int b,
                                                  unsigned gb, int lane)
 {
     const int c = lane & (kTmTU - 1), s = lane >> 3;
     const TmColumn C = S.col[c];
     const int i0 = S.i_begin + S.dir * (b * kTmSB), i = i0 + S.dir * s;
-    const bool live = (c < NL) && (C.i_lo <= i) && (i <= C.i_hi);
+    const bool live = (C.i_lo <= i) && (i <= C.i_hi);
     // Eq. 6 along the slow axis, floor / weight as in Alg. 1 l.9-14
     const double ps = p_of_i(S.s_s, S.s_m, C.rt_s, i);
-    const double jf = floor(ps);
-    const int j = al_to_int(jf);
-    const float u = ceil_weight<INTERP>((float)(ps - jf));
+    const int j = __double2int_rd(ps);                       // floor, saturating
+    const float u = ceil_weight<INTERP>((float)(ps - (double)j));
     const unsigned grp = 0xffu << (8 * s);
     const int jmin = __reduce_min_sync(grp, live ? j : 0x7fffffff);
     const int jmax = __reduce_max_sync(grp, live ? j : -0x7fffffff);
     const bool anylive = jmin != 0x7fffffff;
     // smallest box (4, 6, ..., 12 rows) that holds rows j_min .. j_max + 1
-    const int mi = anylive ? min(max((jmax - jmin + 3) / 2 - 2, 0), (tm_nr<NL>() - 4) / 2) : 0;
+    const int mi = anylive ? min(max((jmax - jmin + 3) / 2 - 2, 0), (kTmNR - 4) / 2) : 0;
     const int box_rows = 4 + 2 * mi;
     const bool fits = live && (j - jmin + 2 <= box_rows);
     if (live && !fits) atomicOr(P.err_flag, 2u);
     // z window of the batch: p_z = s_z + t r_z is monotone in the row, so the extremes sit at the block's end rows
     const double t = __dmul_rn(__dsub_rn((double)i, S.s_m), C.inv_rm);
     const double za = S.s[2] + t * S.rho_first, zb = S.s[2] + t * S.rho_last;
-    const int zlo = __reduce_min_sync(0xffffffffu, al_to_int(floor(fmin(za, zb))));
-    const int zhi = __reduce_max_sync(0xffffffffu, al_to_int(floor(fmax(za, zb))));
+    const int zlo = __reduce_min_sync(0xffffffffu, __double2int_rd(fmin(za, zb)));
+    const int zhi = __reduce_max_sync(0xffffffffu, __double2int_rd(fmax(za, zb)));
     // taps k, k+1 with k = floor(p_z - z0) in [1, W-3] (one spare on either side for fp32 rounding)
     const int z0 = (zlo - 1) & ~3;
     const int need = zhi + 3 - z0;
@@ -229,49 +218,39 @@ __device__ __forceinline__ void tm_produce_batch(TmShared &S, const TmaParams &P
     const int wi = winok ? min(max((need - kTmWMin + kTmWStep - 1) / kTmWStep, 0), kTmWBoxes - 1) : kTmWBoxes - 1;
     const int pitch = kTmWMin + kTmWStep * wi;
     if (!winok && lane == 0) atomicOr(P.err_flag, 1u);
-    const int par = gb & 1;
-    if (s == 0) S.t0[par][c] = winok ? __dmul_rn(__dsub_rn((double)i0, S.s_m), C.inv_rm) : 0.0;
+    const int bp = gb & 1;
+    if (s == 0) S.t0[bp][c] = winok ? __dmul_rn(__dsub_rn((double)i0, S.s_m), C.inv_rm) : 0.0;
     // a window that does not fit is never sampled out of bounds: park every row at p = 4
     if (lane == 0) {
-        S.off[par] = winok ? S.s[2] - (double)z0 : 4.0;
-        S.pitch[par] = (unsigned)(pitch * 4);
+        S.off[bp] = winok ? S.s[2] - (double)z0 : 4.0;
+        S.pitch[bp] = (unsigned)(pitch * 4);
     }
-    // texture columns (NL <= c < NL + NT): row + 1 along the slow axis (the 2 x 2 footprint of texels j, j + 1 is
-    // addressed at their common corner), weight, ray parameter, and z of the block's middle row about an integer
-    // anchor per slice, so that a row's z is one fp32 FMA with operands below 128 whatever the volume size
-    float4 tc = make_float4(-8.0f, 0.0f, 0.0f, 0.0f);
-    double zc = 0.0;
-    if (NT > 0) {
-        const double zmid = S.s[2] + t * S.rho_mid;
-        zc = fmin(fmax(floor(__shfl_sync(0xffffffffu, zmid, 8 * s + NL)), -1.0e6), 1.0e6);
-        const bool tlive = (c >= NL) && (c < NL + NT) && (C.i_lo <= i) && (i <= C.i_hi);
-        tc = make_float4(tlive ? (float)(j + 1) : -8.0f, u, (float)t, (float)(zmid - zc));
-    }
-    uint2 pc;
-    // a column without a sample on this slice reads the two zero rows behind the last stage
-    pc.x = (fits && winok) ? (unsigned)((j - jmin) * pitch * 4) : (unsigned)((kTmSB - s) * tm_stage_floats<NL>() * 4);
-    pc.y = (fits && winok) ? __float_as_uint(u) : 0u;
+    const bool use = fits && winok;
+    const unsigned row_off = (unsigned)((j - jmin) * pitch * 4);
+    const unsigned wbits = use ? __float_as_uint(u) : 0u;
+    // per slice: does it copy a tile, and how large a box (bit 0 = some column live, bits 1.. = box index)
+    const int info = (anylive && winok) ? (1 | (mi << 1)) : 0;
 #pragma unroll
     for (int ss = 0; ss < kTmSB; ++ss) {
-        const int al_s = __shfl_sync(0xffffffffu, (int)anylive, 8 * ss);
+        const int info_s = __shfl_sync(0xffffffffu, info, 8 * ss);
         const int jmin_s = __shfl_sync(0xffffffffu, jmin, 8 * ss);
-        const int i_s = __shfl_sync(0xffffffffu, i, 8 * ss);
-        const int mi_s = __shfl_sync(0xffffffffu, mi, 8 * ss);
-        if (gb > 0 && lane == 0) tm_mbar_wait(&S.empty[ss], (gb - 1) & 1);
-        __syncwarp();
-        if (s == ss) S.stage_col[ss][c] = pc;
-        if (NT > 0 && s == ss && c >= NL && c < NL + NT) S.stage_tex[ss][c - NL] = tc;
-        if (NT > 0 && s == ss && c == NL) S.stage_ti[ss] = make_int2(i, __float_as_int((float)(zc + 1.0)));
+        const int i_s = i0 + S.dir * ss;
+        const int mi_s = info_s >> 1;
+        const unsigned bytes = (info_s & 1) ? (unsigned)((4 + 2 * mi_s) * pitch * 4) : 0u;
+        if (gb > 0) tm_mbar_wait(&S.empty[ss], (gb - 1) & 1);
+        const unsigned phys = (unsigned)(ss * kTmStageFloats * 4);
+        // a column without a sample on this slice reads the two zero rows behind the tiles
+        if (s == ss) S.stage_col[ss][c] = make_uint2(use ? phys + row_off : kTmTileBytes, wbits);
         __syncwarp();
         if (lane == 0) {
-            if (al_s && winok) {
-                tm_mbar_arrive_tx(&S.full[ss], (unsigned)((4 + 2 * mi_s) * pitch * 4));
+            if (bytes) {
+                tm_mbar_arrive_tx(&S.full[ss], bytes);
                 const CUtensorMap *map = &P.map[pass][wi][mi_s];
                 // tensor dimensions are (z, y, x); the slow axis is y for m = x and x for m = y
                 if (pass == 0)
-                    tm_load_3d(map, tiles + ss * tm_stage_floats<NL>(), &S.full[ss], z0, jmin_s, i_s);
+                    tm_load_3d(map, tiles_smem + phys, &S.full[ss], z0, jmin_s, i_s);
                 else
-                    tm_load_3d(map, tiles + ss * tm_stage_floats<NL>(), &S.full[ss], z0, i_s, jmin_s);
+                    tm_load_3d(map, tiles_smem + phys, &S.full[ss], z0, i_s, jmin_s);
             } else {
                 tm_mbar_arrive(&S.full[ss]);
             }
@@ -293,23 +272,24 @@ __device__ __forceinline__ float tm_step_length(const TmShared &S, const TmaPara
     return (float)(P.G.delta * L);
 }
 
-template <int INTERP, int NL, int NT>
-__global__ void __launch_bounds__(kTmThreads, NT > 0 ? 3 : (NL == 6 ? 5 : 4))
+template <int INTERP>
+__global__ void __launch_bounds__(kTmThreads, 4)
 fp_tma_kernel(const __grid_constant__ TmaParams P)
 {
-    constexpr int NB = NL + NT;                            // detector columns per block
     extern __shared__ __align__(128) unsigned char tm_smem_raw[];
-    float *tiles = reinterpret_cast<float *>(tm_smem_raw);                   // kTmSB stages, 128-byte aligned
-    constexpr int kStageFloats = tm_stage_floats<NL>();
-    TmShared &S = *reinterpret_cast<TmShared *>(tm_smem_raw + sizeof(float) * (kTmSB * kStageFloats + 2 * kTmW));
+    float *tiles = reinterpret_cast<float *>(tm_smem_raw);                   // kTmSB stages, then two zero rows; 128-byte aligned
+    TmShared &S = *reinterpret_cast<TmShared *>(tm_smem_raw + kTmTileBytes + sizeof(float) * 2 * kTmW);
 
     const int tid = threadIdx.x, lane = tid & 31;
     // the shuffle tells the compiler that the warp index (and with it the role) is warp-uniform
     const int warp = __shfl_sync(0xffffffffu, tid >> 5, 0);
     const bool producer = warp == kTmConsumers / 32;
-    const int proj = P.ids[blockIdx.z];
+    // blockIdx.x = (detector tile) * group + (projection within the group): see the header
+    const int sel = blockIdx.z * P.group + (int)(blockIdx.x % (unsigned)P.group);
+    if (sel >= P.n_sel) return;                            // the whole block (the last group may be short)
+    const int proj = P.ids[sel];
     const double *g = P.proj[proj].g;
-    const int iu0 = blockIdx.x * NB;
+    const int iu0 = (int)(blockIdx.x / (unsigned)P.group) * kTmTU;
     const int row0 = blockIdx.y * kTmRows;
     // consumer thread t carries detector rows row0 + t and row0 + 128 + t
     const int ct = min(tid, kTmConsumers - 1);
@@ -333,7 +313,6 @@ fp_tma_kernel(const __grid_constant__ TmaParams P)
             S.s[2] = s[2];
             S.rho_first = al_rho(g, P.G, row0, s[2]);
             S.rho_last = al_rho(g, P.G, min(row0 + kTmRows, P.nv) - 1, s[2]);
-            S.rho_mid = al_rho(g, P.G, min(row0 + kTmRows / 2, P.nv - 1), s[2]);
 #pragma unroll
             for (int k = 0; k < kTmSB; ++k) {
                 tm_mbar_init(&S.full[k], 1);
@@ -342,7 +321,7 @@ fp_tma_kernel(const __grid_constant__ TmaParams P)
             asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
         }
     }
-    for (int k = tid; k < 2 * kTmW; k += blockDim.x) tiles[kTmSB * kStageFloats + k] = 0.0f;
+    for (int k = tid; k < 2 * kTmW; k += blockDim.x) tiles[kTmSB * kTmStageFloats + k] = 0.0f;
     __syncthreads();
 
     // Two roles, one code region each (so that no role carries another role's registers); every warp
@@ -350,13 +329,14 @@ fp_tma_kernel(const __grid_constant__ TmaParams P)
     int n_samples = 0;
     if (producer) {
         unsigned gb = 0;                                   // batches issued so far (consumers count alike)
+        const unsigned tiles_smem = tm_smem(tiles);
         for (int pass = 0; pass < 2; ++pass) {
             __syncthreads();                               // every warp is done with the previous pass
-            tm_pass_setup<NL, NT>(S, P, pass, iu0, lane);
+            tm_pass_setup(S, P, pass, iu0, lane);
             __syncthreads();
             if (!S.any) continue;
             const int n_batches = S.n_batches;
-            for (int b = 0; b < n_batches; ++b, ++gb) tm_produce_batch<INTERP, NL, NT>(S, P, tiles, pass, b, gb, lane);
+            for (int b = 0; b < n_batches; ++b, ++gb) tm_produce_batch<INTERP>(S, P, tiles_smem, pass, b, gb, lane);
         }
     } else {
         const double rho0 = al_rho(g, P.G, iv0, S.s[2]), rho1 = al_rho(g, P.G, iv1, S.s[2]);
@@ -364,36 +344,31 @@ fp_tma_kernel(const __grid_constant__ TmaParams P)
         const float2 kMagic2 = make_float2(12582912.0f, 12582912.0f);    // 1.5 * 2^23
         const float2 kNegMagic2 = make_float2(-12582912.0f, -12582912.0f);
         const float2 kNegOne2 = make_float2(-1.0f, -1.0f);
-        float2 acc[NL];
+        float2 acc[kTmTU];
 #pragma unroll
-        for (int c = 0; c < NL; ++c) acc[c] = make_float2(0.0f, 0.0f);
-        // texture columns: r_z of the two rows about the block's middle row, sums
-        float2 tacc[NT > 0 ? NT : 1];
-#pragma unroll
-        for (int k = 0; k < (NT > 0 ? NT : 1); ++k) tacc[k] = make_float2(0.0f, 0.0f);
-        const float2 drho = make_float2((float)(rho0 - S.rho_mid), (float)(rho1 - S.rho_mid));
+        for (int c = 0; c < kTmTU; ++c) acc[c] = make_float2(0.0f, 0.0f);
         unsigned gb = 0;                                   // batches consumed so far
         for (int pass = 0; pass < 2; ++pass) {
             __syncthreads();
             __syncthreads();
             if (!S.any) continue;
             const int n_batches = S.n_batches;
-            float2 dz[NL];                                 // z increment per slice of the two rows, per column
+            float2 dz[kTmTU];                              // z increment per slice of the two rows, per column
 #pragma unroll
-            for (int c = 0; c < NL; ++c) {
+            for (int c = 0; c < kTmTU; ++c) {
                 const double st = fabs(S.col[c].inv_rm);
                 dz[c] = make_float2((float)(rho0 * st), (float)(rho1 * st));
             }
             for (int b = 0; b < n_batches; ++b, ++gb) {
                 const unsigned par = gb & 1;
                 tm_mbar_wait(&S.full[0], par);
-                float2 a[NL];
+                float2 a[kTmTU];
                 unsigned pitchB;
                 {
                     const double off = S.off[par];
                     pitchB = S.pitch[par];
 #pragma unroll
-                    for (int c = 0; c < NL; ++c) {
+                    for (int c = 0; c < kTmTU; ++c) {
                         const double t0 = S.t0[par][c];
                         a[c] = make_float2((float)fma(t0, rho0, off), (float)fma(t0, rho1, off));
                     }
@@ -402,38 +377,17 @@ fp_tma_kernel(const __grid_constant__ TmaParams P)
                 for (int s = 0; s < kTmSB; ++s) {
                     if (s) tm_mbar_wait(&S.full[s], par);
                     const float2 fs = make_float2((float)s, (float)s);
-                    // texture columns of this slice: fetches issued now, used after the tile columns
-                    float4 tv[NT > 0 ? 2 * NT : 1];
-                    float2 td[NT > 0 ? NT : 1];
-                    float tu[NT > 0 ? NT : 1];
-                    if (NT > 0) {
-                        const int2 ti = S.stage_ti[s];
-                        const float zcf = __int_as_float(ti.y);
-#pragma unroll
-                        for (int k = 0; k < NT; ++k) {
-                            const float4 q = S.stage_tex[s][k];
-                            const float2 p = __ffma2_rn(make_float2(q.z, q.z), drho, make_float2(q.w, q.w));
-                            const float2 x = __fadd2_rd(p, kMagic2);
-                            const float2 f = __fadd2_rn(x, kNegMagic2);              // floor(p)
-                            td[k] = __ffma2_rn(f, kNegOne2, p);                      // p - floor(p)
-                            const float2 xc = __fadd2_rn(f, make_float2(zcf, zcf));
-                            tv[2 * k] = tex_gather_layer(P.tex[pass], ti.x, xc.x, q.x);
-                            tv[2 * k + 1] = tex_gather_layer(P.tex[pass], ti.x, xc.y, q.x);
-                            tu[k] = q.y;
-                        }
-                    }
                     uint4 pq2 = make_uint4(0u, 0u, 0u, 0u);
 #pragma unroll
-                    for (int c = 0; c < NL; ++c) {
+                    for (int c = 0; c < kTmTU; ++c) {
                         // one 16-byte broadcast load serves two columns
-                        uint4 pq;
-                        if ((c & 1) == 0) pq = *reinterpret_cast<const uint4 *>(&S.stage_col[s][c]), pq2 = pq;
+                        if ((c & 1) == 0) pq2 = *reinterpret_cast<const uint4 *>(&S.stage_col[s][c]);
                         const uint2 pc = (c & 1) ? make_uint2(pq2.z, pq2.w) : make_uint2(pq2.x, pq2.y);
                         const float2 p = __ffma2_rn(fs, dz[c], a[c]);
                         const float2 x = __fadd2_rd(p, kMagic2);                  // bits = 0x4B400000 + floor(p)
                         const float2 f = __fadd2_rn(x, kNegMagic2);
                         const float2 d = __ffma2_rn(f, kNegOne2, p);              // p - floor(p)
-                        const unsigned rb = tile_bias + pc.x + (unsigned)(s * kStageFloats * 4);
+                        const unsigned rb = tile_bias + pc.x;
                         const unsigned a0 = (__float_as_uint(x.x) << 2) + rb, a1 = (__float_as_uint(x.y) << 2) + rb;
                         const float2 v00 = make_float2(al_lds(a0), al_lds(a1));
                         const float2 v01 = make_float2(al_lds(a0 + 4u), al_lds(a1 + 4u));
@@ -446,18 +400,6 @@ fp_tma_kernel(const __grid_constant__ TmaParams P)
                         const float2 t1 = __ffma2_rn(wz, __ffma2_rn(v10, kNegOne2, v11), v10);   // row j + 1
                         acc[c] = __fadd2_rn(acc[c], __ffma2_rn(make_float2(uy, uy), __ffma2_rn(t0, kNegOne2, t1), t0));
                     }
-                    if (NT > 0) {
-#pragma unroll
-                        for (int k = 0; k < NT; ++k) {
-                            // gather order: w = (k, j), z = (k + 1, j), x = (k, j + 1), y = (k + 1, j + 1)
-                            const float wa = ceil_weight<INTERP>(td[k].x), wb = ceil_weight<INTERP>(td[k].y);
-                            const float4 va = tv[2 * k], vb = tv[2 * k + 1];
-                            const float a0 = fmaf(wa, va.z - va.w, va.w), a1 = fmaf(wa, va.y - va.x, va.x);
-                            const float b0 = fmaf(wb, vb.z - vb.w, vb.w), b1 = fmaf(wb, vb.y - vb.x, vb.x);
-                            tacc[k].x += fmaf(tu[k], a1 - a0, a0);
-                            tacc[k].y += fmaf(tu[k], b1 - b0, b0);
-                        }
-                    }
                     __syncwarp();
                     if (lane == 0) tm_mbar_arrive(&S.empty[s]);
                 }
@@ -469,27 +411,20 @@ fp_tma_kernel(const __grid_constant__ TmaParams P)
             const int iv = row0 + h * kTmConsumers + tid;
             if (iv >= P.nv) continue;
             const double rho = h ? rho1 : rho0;
-            float o[NB];
+            float o[kTmTU];
 #pragma unroll
-            for (int c = 0; c < NL; ++c) o[c] = tm_step_length(S, P, c, rho) * (h ? acc[c].y : acc[c].x);
-#pragma unroll
-            for (int k = 0; k < NT; ++k) o[NL + k] = tm_step_length(S, P, NL + k, rho) * (h ? tacc[k].y : tacc[k].x);
+            for (int c = 0; c < kTmTU; ++c) o[c] = tm_step_length(S, P, c, rho) * (h ? acc[c].y : acc[c].x);
             float *dst = P.out + ((size_t)proj * P.nv + iv) * P.nu + iu0;
-            if (NB == 8 && P.out_vec && iu0 + NB <= P.nu) {
+            if (P.out_vec && iu0 + kTmTU <= P.nu) {
                 reinterpret_cast<float4 *>(dst)[0] = make_float4(o[0], o[1], o[2], o[3]);
-                reinterpret_cast<float4 *>(dst)[1] = make_float4(o[NB - 4], o[NB - 3], o[NB - 2], o[NB - 1]);
-            } else if (NB == 6 && P.out_vec && iu0 + NB <= P.nu) {
-                // 6 columns = 24 bytes: the row start is 8-byte aligned
-                reinterpret_cast<float2 *>(dst)[0] = make_float2(o[0], o[1]);
-                reinterpret_cast<float2 *>(dst)[1] = make_float2(o[2], o[3]);
-                reinterpret_cast<float2 *>(dst)[2] = make_float2(o[NB - 2], o[NB - 1]);
+                reinterpret_cast<float4 *>(dst)[1] = make_float4(o[4], o[5], o[6], o[7]);
             } else {
 #pragma unroll
-                for (int c = 0; c < NB; ++c)
+                for (int c = 0; c < kTmTU; ++c)
                     if (iu0 + c < P.nu) dst[c] = o[c];
             }
             if (P.sample_count) {
-                for (int c = 0; c < NB; ++c)
+                for (int c = 0; c < kTmTU; ++c)
                     if (iu0 + c < P.nu) {
                         const RaySetup R = ray_setup(g, P.G, iu0 + c, iv);
                         n_samples += max(R.i_last - R.i_first + 1, 0);
@@ -500,7 +435,6 @@ fp_tma_kernel(const __grid_constant__ TmaParams P)
     if (P.sample_count) block_count_samples(P.sample_count, n_samples);
 }
 
-template <int NL>
-constexpr size_t tma_smem_bytes() { return sizeof(float) * (kTmSB * tm_stage_floats<NL>() + 2 * kTmW) + sizeof(TmShared); }
+constexpr size_t tma_smem_bytes() { return kTmTileBytes + sizeof(float) * 2 * kTmW + sizeof(TmShared); }
 
 }  // namespace fpk

@@ -18,7 +18,7 @@ LIB_PATH = os.path.join(_HERE, "libfp.so")
 FP_OK = 0
 STATUS = {0: "FP_OK", 1: "FP_ERR_INVALID_ARG", 2: "FP_ERR_CUDA", 3: "FP_ERR_OOM", 4: "FP_ERR_UNSUPPORTED"}
 
-OPT_KERNEL, OPT_VOLATILE, OPT_INTERP, OPT_PERMUTED_COPY, OPT_COUNT_SAMPLES, OPT_FOV_CYLINDER, OPT_TEX_SHARE, OPT_TEX_COLUMNS = 1, 2, 3, 4, 5, 6, 7, 8
+OPT_KERNEL, OPT_VOLATILE, OPT_INTERP, OPT_PERMUTED_COPY, OPT_COUNT_SAMPLES, OPT_FOV_CYLINDER = 1, 2, 3, 4, 5, 6
 KERNEL_AUTO, KERNEL_DIRECT, KERNEL_ALIGNED, KERNEL_TMA, KERNEL_TEX, KERNEL_HWLIN = 0, 1, 2, 3, 4, 5
 INTERP_LINEAR, INTERP_SPLINE = 0, 1
 
