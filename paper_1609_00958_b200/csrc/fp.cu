@@ -28,7 +28,7 @@ struct fp_ctx {
     int opt_permuted = 1;
     int opt_count = 1;
     int opt_fov = 0;
-    int opt_group = 4;                         // projections per launch-order group of fp_tma_kernel
+    int opt_group = 8;                         // projections per launch-order group of fp_tma_kernel
     // layout stage: y-fastest copy [nz][nx][ny] for z-driven rays
     float *vol_perm = nullptr;
     const float *perm_src = nullptr;
@@ -695,7 +695,10 @@ extern "C" fp_status fp_project(fp_ctx *c, const float *vol_dev, int n_proj, con
         A.nv = nv;
         A.n_sel = (int)ids_al.size();
         A.fov = c->opt_fov;
-        dim3 grid((unsigned)((nu + kAlTU - 1) / kAlTU), (unsigned)((nv + kAlTV - 1) / kAlTV), (unsigned)ids_al.size());
+        A.out_vec = ((uintptr_t)out_dev & 15) == 0 && (nu & 3) == 0;
+        A.group = std::max(1, std::min(c->opt_group, (int)ids_al.size()));
+        dim3 grid((unsigned)((nu + kAlTU - 1) / kAlTU * A.group), (unsigned)((nv + kAlTV - 1) / kAlTV),
+                  (unsigned)((ids_al.size() + A.group - 1) / A.group));
         s = c->opt_interp == FP_INTERP_SPLINE ? launch_aligned<1>(c, A, w_al, grid, st)
                                               : launch_aligned<0>(c, A, w_al, grid, st);
         if (s != FP_OK) return s;

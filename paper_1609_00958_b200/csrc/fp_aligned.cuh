@@ -37,6 +37,8 @@ struct AlignedParams {
     unsigned int *err_flag;            // set to 1 if a staging window would overflow
     int nu, nv, n_sel;
     int fov;                           // 1: the volume is zero outside the inscribed cylinder about z (FP_OPT_FOV_CYLINDER)
+    int out_vec;                       // 1: out is 16-byte aligned and nu % 4 == 0 (vector stores allowed)
+    int group;                         // projections whose blocks are interleaved in launch order (>= 1), as in fp_tma.cuh
 };
 
 struct AlColumn {          // per detector column, constant over the slice loop
@@ -176,9 +178,13 @@ fp_aligned_kernel(const __grid_constant__ AlignedParams P)
     float *lines = reinterpret_cast<float *>(al_smem_raw + sizeof(AlShared));
 
     const int tid = threadIdx.x;
-    const int proj = P.ids[blockIdx.z];
+    // blockIdx.x = (detector tile) * group + (projection within the group): neighbouring poses sweep the volume
+    // in step and share its rows through L2 (fp_tma.cuh)
+    const int sel = blockIdx.z * P.group + (int)(blockIdx.x % (unsigned)P.group);
+    if (sel >= P.n_sel) return;                            // the whole block (the last group may be short)
+    const int proj = P.ids[sel];
     const double *g = P.proj[proj].g;
-    const int iu0 = blockIdx.x * kAlTU;
+    const int iu0 = (int)(blockIdx.x / (unsigned)P.group) * kAlTU;
     const int row0 = blockIdx.y * kAlTV;
     const int iv = min(row0 + tid, P.nv - 1);
 
@@ -363,7 +369,7 @@ fp_aligned_kernel(const __grid_constant__ AlignedParams P)
             o[c] = (float)(P.G.delta * L) * (acc[c].x + acc[c].y);
         }
         float *dst = P.out + ((size_t)proj * P.nv + iv) * P.nu + iu0;
-        if ((P.nu & 3) == 0 && iu0 + kAlTU <= P.nu) {
+        if (P.out_vec && iu0 + kAlTU <= P.nu) {
             reinterpret_cast<float4 *>(dst)[0] = make_float4(o[0], o[1], o[2], o[3]);
             reinterpret_cast<float4 *>(dst)[1] = make_float4(o[4], o[5], o[6], o[7]);
         } else {
