@@ -241,7 +241,7 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--kernel", type=int, default=0, help="FP_OPT_KERNEL value (0 = auto)")
-    ap.add_argument("--group", type=int, default=-1)
+    ap.add_argument("--group", type=int, default=-1, help="FP_OPT_GROUP (-1 = library default)")
     ap.add_argument("--op", default="project", choices=["project", "backproject"],
                     help="project: the headline forward projector; backproject: its exact transpose (SURVEY 8(f) #2)")
     ap.add_argument("--interp", default="linear", choices=["linear", "spline"],
@@ -278,7 +278,7 @@ def main():
     interp = fp.INTERP_SPLINE if args.interp == "spline" else fp.INTERP_LINEAR
     P.set_option(fp.OPT_INTERP, interp)
     if args.group >= 0:
-        P.set_option(100, args.group)
+        P.set_option(fp.OPT_GROUP, args.group)
     if cfg.cylinder:
         P.set_option(fp.OPT_FOV_CYLINDER, 1)       # the volume is zero outside the inscribed cylinder
     stream = torch.cuda.current_stream()

@@ -32,6 +32,9 @@
  *     (and the degenerate ray r = 0) write +0.0f.
  *   - Streams: every kernel and copy is enqueued on the given stream; fp_project does not
  *     synchronise the host with the device.  Outputs are valid once the stream reaches that point.
+ *     A context owns one set of workspaces: a call on another stream than the context's previous call
+ *     first waits (on the device) for that call to end, so calls on one context never overlap.  Use one
+ *     context per stream for concurrent projections.
  *   - Ownership: the caller owns the volume, the geometry and the outputs.  The library owns
  *     the context, its internal volume copies and workspaces (freed by fp_destroy).
  *   - Errors: status codes only, nothing is thrown.  fp_last_error(ctx) holds the text of the
@@ -101,7 +104,15 @@ enum {
      * the slices of a ray on which every tap lies outside that cylinder; for such a volume the result is the
      * same sum.  The direct kernel ignores the option; fp_last_sample_count keeps counting the box samples.
      * Default 0. */
-    FP_OPT_FOV_CYLINDER = 6
+    FP_OPT_FOV_CYLINDER = 6,
+    /* Projections per launch-order group of the aligned / TMA kernels (1 .. 64, default 8): the thread blocks of
+     * the same detector tile of `group` consecutive poses of a call start together and sweep the volume in step,
+     * so that neighbouring poses of an orbit read the volume rows they share from L2 instead of DRAM.  A tuning
+     * knob only: results do not depend on it. */
+    FP_OPT_GROUP = 7,
+    /* TEST HOOK, not for production: 1 sends every aligned pose to FP_KERNEL_TMA whether the host plan says its
+     * tiles fit or not, so that the kernel's own bound checks (fp_check) can be exercised. */
+    FP_OPT_TEST_FORCE_TMA = 100
 };
 
 enum { FP_KERNEL_AUTO = 0, FP_KERNEL_DIRECT = 1, FP_KERNEL_ALIGNED = 2, FP_KERNEL_TMA = 3, FP_KERNEL_TEX = 4, FP_KERNEL_HWLIN = 5 };
@@ -175,8 +186,21 @@ fp_status fp_ray_ranges(fp_ctx *ctx, int n_proj, const double *geom_host, int nu
  * fp_last_sample_count: number of samples (visited slices summed over rays) of the most recent
  * fp_project / fp_project_host on this context; synchronises the stream that call used.
  * This is the unit of the paper's "memory access rate" = 16 B x samples / time.
+ * Returns FP_ERR_UNSUPPORTED if fp_check would (and clears that flag), FP_ERR_INVALID_ARG if the most recent
+ * call did not count (FP_OPT_COUNT_SAMPLES = 0).
  */
 fp_status fp_last_sample_count(fp_ctx *ctx, unsigned long long *n);
+
+/*
+ * fp_check: synchronises the stream of the most recent call on this context and reports whether any sampling
+ * kernel since the last fp_check / fp_last_sample_count found that the host plan had under-sized a staging
+ * window or a row tile of the aligned / TMA kernels (the plan bounds them by geometry; the kernels verify the
+ * bound and raise a flag instead of reading out of bounds).  FP_OK: every projection written since the last
+ * check is valid.  FP_ERR_UNSUPPORTED: some are not -- repeat those calls with FP_OPT_KERNEL = FP_KERNEL_DIRECT
+ * (fp_project_host does this by itself).  The flag is cleared by the call.  fp_project cannot report this
+ * itself because it never synchronises.
+ */
+fp_status fp_check(fp_ctx *ctx);
 
 /*
  * fp_plan: the host-side plan fp_project makes for ONE pose (no device needed, nothing is launched):

@@ -63,6 +63,14 @@ def lib():
         L.jo_backproject.argtypes = [dp, cip, ctypes.c_double, dp, dp, ctypes.c_int, ctypes.c_int, ctypes.c_int,
                                      ctypes.c_int, dp]
         L.jo_backproject.restype = None
+        L.jo_ray_grid_axis.argtypes = [fp, cip, dp, dp, ctypes.c_int, ctypes.c_int, dp, ip, dp]
+        L.jo_ray_grid_axis.restype = None
+        L.jo_project_rays_axis.argtypes = [fp, cip, ctypes.c_double, dp, dp, ctypes.c_int, ctypes.c_long, ip, ip,
+                                           dp, ip, dp]
+        L.jo_project_rays_axis.restype = None
+        L.jo_backproject_voxels.argtypes = [dp, cip, ctypes.c_double, dp, dp, ctypes.c_int, ctypes.c_int,
+                                            ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_long, ip, dp]
+        L.jo_backproject_voxels.restype = None
         _lib = L
     return _lib
 
@@ -99,6 +107,19 @@ def ray_grid(vol, s, d, kernel: int = KERNEL_LIN):
                       ctypes.byref(L), _dptr(mg))
     return dict(value=val.value, m=int(mfl[0]), i_first=int(mfl[1]), i_last=int(mfl[2]),
                 L=L.value, margins=(float(mg[0]), float(mg[1])))
+
+
+def ray_grid_axis(vol, s, d, m: int, kernel: int = KERNEL_LIN):
+    """One ray in grid coordinates with the driving axis given (jo_ray_grid_axis)."""
+    v, n = _vol(vol)
+    s = np.ascontiguousarray(s, dtype=np.float64)
+    d = np.ascontiguousarray(d, dtype=np.float64)
+    val = ctypes.c_double()
+    L = ctypes.c_double()
+    mfl = np.zeros(3, dtype=np.int32)
+    lib().jo_ray_grid_axis(_fptr(v), n, _dptr(s), _dptr(d), kernel, int(m), ctypes.byref(val), _iptr(mfl),
+                           ctypes.byref(L))
+    return dict(value=val.value, m=int(mfl[0]), i_first=int(mfl[1]), i_last=int(mfl[2]), L=L.value)
 
 
 def ray_definition(vol, s, d, kernel: int = KERNEL_LIN) -> float:
@@ -141,6 +162,25 @@ def project_rays(vol, voxel_size, origin, geom, ray_ids, kernel: int = KERNEL_LI
         with ThreadPoolExecutor(max_workers=threads) as ex:
             list(ex.map(lambda lo: run(lo, min(nr, lo + chunk)), range(0, nr, chunk)))
     return values, mfl, pathlen, margins
+
+
+def project_rays_axis(vol, voxel_size, origin, geom, ray_ids, axis, kernel: int = KERNEL_LIN):
+    """project_rays with the driving axis GIVEN per ray (jo_ray_grid_axis; reading #8: the parity
+    harness evaluates near-tie rays along the axis the GPU took).  Returns (values, mfl, pathlen)."""
+    v, n = _vol(vol)
+    origin = np.ascontiguousarray(origin, dtype=np.float64)
+    geom = np.ascontiguousarray(geom, dtype=np.float64).reshape(-1, 12)
+    ids = np.ascontiguousarray(ray_ids, dtype=np.int32).reshape(-1, 3)
+    ax = np.ascontiguousarray(axis, dtype=np.int32).reshape(-1)
+    nr = ids.shape[0]
+    assert ax.shape[0] == nr
+    values = np.zeros(nr, dtype=np.float64)
+    mfl = np.zeros((nr, 3), dtype=np.int32)
+    pathlen = np.zeros(nr, dtype=np.float64)
+    if nr:
+        lib().jo_project_rays_axis(_fptr(v), n, float(voxel_size), _dptr(origin), _dptr(geom), kernel, nr,
+                                   _iptr(ids), _iptr(ax), _dptr(values), _iptr(mfl), _dptr(pathlen))
+    return values, mfl, pathlen
 
 
 def project_block(vol, voxel_size, origin, geom_row, iu0, iu1, iv0, iv1, kernel: int = KERNEL_LIN):
@@ -211,6 +251,36 @@ def backproject(proj, shape, voxel_size, origin, geom, kernel: int = KERNEL_LIN,
     with ThreadPoolExecutor(max_workers=threads) as ex:
         parts = list(ex.map(lambda k: run(int(cuts[k]), int(cuts[k + 1])), range(threads)))
     return sum(parts[1:], parts[0])
+
+
+def backproject_voxels(proj, shape, voxel_size, origin, geom, voxels, halfwin: int, kernel: int = KERNEL_LIN,
+                       threads: int = 1):
+    """(A^T proj)[v] for the listed voxels[n][3] = (ix, iy, iz) by the definition of the transpose
+    (jo_backproject_voxels); halfwin = half width in pixels of the detector window visited around each voxel's
+    projection.  Returns f64[n]."""
+    y = np.ascontiguousarray(proj, dtype=np.float64)
+    n_proj, nv, nu = y.shape
+    geom = np.ascontiguousarray(geom, dtype=np.float64).reshape(-1, 12)
+    assert geom.shape[0] == n_proj
+    origin = np.ascontiguousarray(origin, dtype=np.float64)
+    vox = np.ascontiguousarray(voxels, dtype=np.int32).reshape(-1, 3)
+    out = np.zeros(vox.shape[0], dtype=np.float64)
+    n = (ctypes.c_int * 3)(*[int(k) for k in shape])
+    lib()
+
+    def run(lo, hi):
+        if hi > lo:
+            lib().jo_backproject_voxels(_dptr(y), n, float(voxel_size), _dptr(origin), _dptr(geom), kernel, n_proj, nu,
+                                        nv, int(halfwin), hi - lo, _iptr(vox[lo:hi]), _dptr(out[lo:hi]))
+
+    nq = vox.shape[0]
+    if threads <= 1 or nq < 4 * threads:
+        run(0, nq)
+    else:
+        chunk = max(1, (nq + 8 * threads - 1) // (8 * threads))
+        with ThreadPoolExecutor(max_workers=threads) as ex:
+            list(ex.map(lambda lo: run(lo, min(nq, lo + chunk)), range(0, nq, chunk)))
+    return out
 
 
 def host_cores() -> int:

@@ -320,3 +320,147 @@ void jo_backproject(const double *proj, const int n[3], double delta, const doub
                 }
             }
 }
+
+/*
+ * jo_ray_grid_axis: the step-by-step form of jo_ray_grid with the driving axis GIVEN instead of
+ * chosen by Eq. 2.  The paper is silent on exact ties |r_a| = |r_b| (DESIGN.md
+ * reading #8): both axes give a valid Joseph sum, and they differ.  The parity harness uses this
+ * routine only for rays whose two largest |r_a| agree to within 1e-9 relative and for which the
+ * GPU took the other axis: the GPU value must then match the sum along ITS axis.  Same formulas as
+ * jo_ray_grid (Eqs. 4-6, Alg. 1 l.6-20) with m := m_forced; r_m must be non-zero.
+ *   mfl = { m_forced, i_first, i_last }
+ */
+void jo_ray_grid_axis(const float *vol, const int n[3], const double s[3], const double d[3],
+                      int kernel, int m_forced, double *value_grid, int32_t mfl[3], double *L_out)
+{
+    double r[3], rt[3], L, acc = 0.0;
+    int a, m = m_forced, t1, t2, i, i_first = 0, i_last = -1, found = 0;
+    *value_grid = 0.0;
+    mfl[0] = m; mfl[1] = 0; mfl[2] = -1;
+    if (L_out) *L_out = 0.0;
+    if (m < 0 || m > 2) return;
+    for (a = 0; a < 3; ++a) r[a] = d[a] - s[a];            /* Eq. 1 */
+    if (r[m] == 0.0) return;
+    for (a = 0; a < 3; ++a) rt[a] = r[a] / r[m];           /* Eq. 4 with the given axis */
+    rt[m] = 1.0;
+    L = sqrt(rt[0] * rt[0] + rt[1] * rt[1] + rt[2] * rt[2]);
+    if (L_out) *L_out = L;
+    t1 = (m + 1) % 3;
+    t2 = (m + 2) % 3;
+    for (i = 0; i < n[m]; ++i) {                           /* step 6 */
+        double p1 = jo_pt(s, rt, m, t1, i), p2 = jo_pt(s, rt, m, t2, i);
+        if ((-1.0 < p1) && (p1 < (double)n[t1]) && (-1.0 < p2) && (p2 < (double)n[t2])) {
+            if (!found) { i_first = i; found = 1; }
+            i_last = i;
+        }
+    }
+    if (!found) return;
+    mfl[1] = i_first;
+    mfl[2] = i_last;
+    for (i = i_first; i <= i_last; ++i) {                  /* steps 7-8 */
+        double p[3], w0[3], w1[3];
+        long fl[3];
+        int b;
+        p[m] = (double)i;
+        p[t1] = jo_pt(s, rt, m, t1, i);
+        p[t2] = jo_pt(s, rt, m, t2, i);
+        for (a = 0; a < 3; ++a) {
+            double f = floor(p[a]);
+            fl[a] = (long)f;
+            w0[a] = jo_w(kernel, p[a] - f);
+            w1[a] = 1.0 - w0[a];
+        }
+        for (a = 0; a < 2; ++a)
+            for (b = 0; b < 2; ++b) {
+                long idx[3];
+                idx[m] = fl[m];
+                idx[t1] = fl[t1] + a;
+                idx[t2] = fl[t2] + b;
+                acc += jo_vox(vol, n, idx[0], idx[1], idx[2]) * (a ? w1[t1] : w0[t1]) * (b ? w1[t2] : w0[t2]);
+            }
+    }
+    *value_grid = L * acc;
+}
+
+/* jo_project_rays_axis: jo_project_rays with a driving axis given per ray (axis[q] in 0..2). */
+void jo_project_rays_axis(const float *vol, const int n[3], double delta, const double origin[3],
+                          const double *geom, int kernel, long n_rays, const int32_t *ray_ids,
+                          const int32_t *axis, double *values, int32_t *mfl, double *pathlen)
+{
+    long q;
+    for (q = 0; q < n_rays; ++q) {
+        double s[3], d[3], v, L;
+        int32_t t[3];
+        const double *g = geom + 12 * (size_t)ray_ids[3 * q];
+        jo_pixel_to_grid(g, delta, origin, ray_ids[3 * q + 2], ray_ids[3 * q + 1], s, d);
+        jo_ray_grid_axis(vol, n, s, d, kernel, axis[q], &v, t, &L);
+        values[q] = delta * v;
+        if (mfl) { mfl[3 * q] = t[0]; mfl[3 * q + 1] = t[1]; mfl[3 * q + 2] = t[2]; }
+        if (pathlen) pathlen[q] = delta * L * (double)(t[2] - t[1] + 1);
+    }
+}
+
+/*
+ * jo_backproject_voxels: (A^T proj)[v] for a LIST of voxels, by the definition of the transpose,
+ * (A^T y)[v] = sum_rays y[ray] * (A e_v)[ray].
+ * With e_v the unit volume at voxel v = (ix, iy, iz), a ray sees it on exactly one slice, i = v_m,
+ * with the weight  delta * ||r~|| * H(p_t1(i) - v_t1) * H(p_t2(i) - v_t2),  H the hat of
+ * jo_ray_definition -- no floor, no tap list.  Only the pixels within `halfwin` of the voxel
+ * centre's projection onto the detector are visited (every other ray passes more than one voxel
+ * away from v on slice v_m and has weight zero; the caller chooses halfwin and the tests check it
+ * against the full jo_backproject).
+ *   vox   [n_vox][3] = ix, iy, iz;     out [n_vox]  (overwritten)
+ */
+void jo_backproject_voxels(const double *proj, const int n[3], double delta, const double origin[3],
+                           const double *geom, int kernel, int n_proj, int nu, int nv, int halfwin,
+                           long n_vox, const int32_t *vox, double *out)
+{
+    long q;
+    int p;
+    for (q = 0; q < n_vox; ++q) {
+        const int32_t *v = vox + 3 * q;
+        double acc = 0.0;
+        out[q] = 0.0;
+        if (v[0] < 0 || v[1] < 0 || v[2] < 0 || v[0] >= n[0] || v[1] >= n[1] || v[2] >= n[2])
+            continue;
+        for (p = 0; p < n_proj; ++p) {
+            const double *g = geom + 12 * (size_t)p;
+            double x[3], e[3], nrm[3], uu = 0.0, vv = 0.0, uv = 0.0, den = 0.0, num = 0.0, lam, h[3], bu = 0.0, bv = 0.0, det;
+            int a, iu, iv, cu, cv;
+            /* voxel centre in world units; intersect the line source -> centre with the detector plane */
+            for (a = 0; a < 3; ++a) x[a] = origin[a] + delta * (double)v[a];
+            nrm[0] = g[7] * g[11] - g[8] * g[10];
+            nrm[1] = g[8] * g[9] - g[6] * g[11];
+            nrm[2] = g[6] * g[10] - g[7] * g[9];
+            for (a = 0; a < 3; ++a) { e[a] = x[a] - g[a]; den += nrm[a] * e[a]; num += nrm[a] * (g[3 + a] - g[a]); }
+            if (den == 0.0) continue;
+            lam = num / den;
+            if (!(lam > 0.0)) continue;
+            for (a = 0; a < 3; ++a) h[a] = g[a] + lam * e[a] - g[3 + a];     /* hit point relative to det_origin */
+            for (a = 0; a < 3; ++a) { uu += g[6 + a] * g[6 + a]; vv += g[9 + a] * g[9 + a]; uv += g[6 + a] * g[9 + a];
+                                      bu += g[6 + a] * h[a]; bv += g[9 + a] * h[a]; }
+            det = uu * vv - uv * uv;
+            if (det == 0.0) continue;
+            cu = (int)floor((bu * vv - bv * uv) / det + 0.5);
+            cv = (int)floor((bv * uu - bu * uv) / det + 0.5);
+            for (iv = cv - halfwin; iv <= cv + halfwin; ++iv)
+                for (iu = cu - halfwin; iu <= cu + halfwin; ++iu) {
+                    double s[3], d[3], rt[3], L, x1, x2, h1, h2;
+                    int m, t1, t2, i;
+                    if (iu < 0 || iv < 0 || iu >= nu || iv >= nv) continue;
+                    jo_pixel_to_grid(g, delta, origin, iu, iv, s, d);
+                    if (!jo_setup(s, d, &m, rt, &L)) continue;
+                    t1 = (m + 1) % 3;
+                    t2 = (m + 2) % 3;
+                    i = v[m];
+                    x1 = fabs(jo_pt(s, rt, m, t1, i) - (double)v[t1]);
+                    x2 = fabs(jo_pt(s, rt, m, t2, i) - (double)v[t2]);
+                    h1 = x1 < 1.0 ? jo_w(kernel, x1) : 0.0;
+                    h2 = x2 < 1.0 ? jo_w(kernel, x2) : 0.0;
+                    acc += delta * L * h1 * h2
+                           * proj[((size_t)p * (size_t)nv + (size_t)iv) * (size_t)nu + (size_t)iu];
+                }
+        }
+        out[q] = acc;
+    }
+}

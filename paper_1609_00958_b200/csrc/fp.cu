@@ -28,7 +28,8 @@ struct fp_ctx {
     int opt_permuted = 1;
     int opt_count = 1;
     int opt_fov = 0;
-    int opt_group = 8;                         // projections per launch-order group of fp_tma_kernel
+    int opt_group = 8;                         // projections per launch-order group of the aligned / TMA kernels
+    int opt_force_tma = 0;                     // test hook: every aligned pose goes to fp_tma_kernel whether it fits or not
     // layout stage: y-fastest copy [nz][nx][ny] for z-driven rays
     float *vol_perm = nullptr;
     const float *perm_src = nullptr;
@@ -52,6 +53,8 @@ struct fp_ctx {
     bool arr_valid[3] = {false, false, false};
     int n_sm = 0;
     cudaStream_t last_stream = nullptr;
+    cudaEvent_t ev_last = nullptr;                   // end of the most recent call: a call on another stream waits for it
+    bool ev_valid = false;
     bool counted = false;
     int last_launches = 0;
     // fp_project_host workspaces
@@ -84,6 +87,45 @@ static fp_status cuda_fail(fp_ctx *c, cudaError_t e, const char *what)
         cudaError_t e_ = (call);                                       \
         if (e_ != cudaSuccess) return cuda_fail((ctx), e_, #call);     \
     } while (0)
+
+// The per-context workspaces (geometry rows, projection ids, counters) are rewritten by every call in stream
+// order.  A call on another stream than the previous one first waits for that call's end, so that two streams
+// never race on them (the calls are then serialised: use one context per stream for concurrency).
+static fp_status enter_stream(fp_ctx *c, cudaStream_t st)
+{
+    if (c->ev_valid && st != c->last_stream) FP_CUDA(c, cudaStreamWaitEvent(st, c->ev_last, 0));
+    if (!c->count_dev) {
+        FP_CUDA(c, cudaMalloc(&c->count_dev, 2 * sizeof(unsigned long long)));
+        FP_CUDA(c, cudaMemsetAsync(c->count_dev, 0, 2 * sizeof(unsigned long long), st));
+    }
+    return FP_OK;
+}
+
+static fp_status leave_stream(fp_ctx *c, cudaStream_t st)
+{
+    if (!c->ev_last) FP_CUDA(c, cudaEventCreateWithFlags(&c->ev_last, cudaEventDisableTiming));
+    FP_CUDA(c, cudaEventRecord(c->ev_last, st));
+    c->ev_valid = true;
+    c->last_stream = st;
+    return FP_OK;
+}
+
+// Synchronises the stream of the most recent call and reads { sample count, error flag }; a raised flag (a
+// staging window or row tile of the aligned / TMA kernels did not fit: the host plan was too small and the
+// affected rays hold wrong values) is cleared by the read.
+static fp_status read_counters(fp_ctx *c, unsigned long long h[2])
+{
+    h[0] = h[1] = 0;
+    if (!c->count_dev) return FP_OK;
+    FP_CUDA(c, cudaStreamSynchronize(c->last_stream));
+    FP_CUDA(c, cudaMemcpy(h, c->count_dev, 2 * sizeof(unsigned long long), cudaMemcpyDeviceToHost));
+    if (h[1] != 0) FP_CUDA(c, cudaMemset(c->count_dev + 1, 0, sizeof(unsigned long long)));
+    return FP_OK;
+}
+
+static const char *kPlanError =
+    "a staging window or row tile of the aligned / TMA kernel did not fit (host plan too small): the projections "
+    "written since the last check are invalid; repeat the call with FP_OPT_KERNEL = FP_KERNEL_DIRECT";
 
 static size_t n_voxels(const fp_ctx *c) { return (size_t)c->G.n[0] * c->G.n[1] * c->G.n[2]; }
 
@@ -131,6 +173,7 @@ extern "C" fp_status fp_destroy(fp_ctx *c)
     cudaFree(c->vol_perm);
     cudaFree(c->proj_dev);
     cudaFree(c->count_dev);
+    if (c->ev_last) cudaEventDestroy(c->ev_last);
     cudaFree(c->ids_dev);
     cudaFree(c->hvol_dev);
     for (int a = 0; a < 3; ++a) {
@@ -169,7 +212,11 @@ extern "C" fp_status fp_set_option(fp_ctx *c, int key, int value)
         return FP_OK;
     case FP_OPT_COUNT_SAMPLES: c->opt_count = value != 0; return FP_OK;
     case FP_OPT_FOV_CYLINDER: c->opt_fov = value != 0; return FP_OK;
-    case 100: c->opt_group = value; return FP_OK;   // DEV
+    case FP_OPT_GROUP:
+        if (value < 1 || value > 64) return fail(c, FP_ERR_INVALID_ARG, "FP_OPT_GROUP must be 1 .. 64");
+        c->opt_group = value;
+        return FP_OK;
+    case FP_OPT_TEST_FORCE_TMA: c->opt_force_tma = value != 0; return FP_OK;
     }
     return fail(c, FP_ERR_INVALID_ARG, "unknown option key");
 }
@@ -184,6 +231,8 @@ extern "C" fp_status fp_get_option(fp_ctx *c, int key, int *value)
     case FP_OPT_PERMUTED_COPY: *value = c->opt_permuted; return FP_OK;
     case FP_OPT_COUNT_SAMPLES: *value = c->opt_count; return FP_OK;
     case FP_OPT_FOV_CYLINDER: *value = c->opt_fov; return FP_OK;
+    case FP_OPT_GROUP: *value = c->opt_group; return FP_OK;
+    case FP_OPT_TEST_FORCE_TMA: *value = c->opt_force_tma; return FP_OK;
     }
     return fail(c, FP_ERR_INVALID_ARG, "unknown option key");
 }
@@ -578,9 +627,10 @@ extern "C" fp_status fp_project(fp_ctx *c, const float *vol_dev, int n_proj, con
     if (s != FP_OK) return s;
     cudaStream_t st = (cudaStream_t)stream;
     c->last_launches = 0;
-    c->last_stream = st;
     c->counted = false;
     if (n_proj == 0) return FP_OK;
+    s = enter_stream(c, st);
+    if (s != FP_OK) return s;
 
     // plan: which kernel takes which projection
     std::vector<int> ids_al, ids_di, ids_tm, ids_tx;
@@ -593,7 +643,7 @@ extern "C" fp_status fp_project(fp_ctx *c, const float *vol_dev, int n_proj, con
         }
         int rows = 0;
         const int w = c->opt_kernel == FP_KERNEL_DIRECT ? 0 : plan_aligned(c, vol_dev, geom + 12 * (size_t)p, nu, nv, &rows);
-        if (fits_tma(w, rows) && c->opt_kernel != FP_KERNEL_ALIGNED) {
+        if ((fits_tma(w, rows) || (c->opt_force_tma && w > 0)) && c->opt_kernel != FP_KERNEL_ALIGNED) {
             ids_tm.push_back(p);                       // fits the TMA-fed kernel's tile
         } else if (w > 0 && w <= kAlignedMaxW) {
             ids_al.push_back(p);
@@ -638,8 +688,8 @@ extern "C" fp_status fp_project(fp_ctx *c, const float *vol_dev, int n_proj, con
         FP_CUDA(c, cudaMemcpyAsync(c->ids_dev + 3 * c->ids_cap, ids_tx.data(), sizeof(int) * ids_tx.size(),
                                    cudaMemcpyHostToDevice, st));
 
-    if (!c->count_dev) FP_CUDA(c, cudaMalloc(&c->count_dev, 2 * sizeof(unsigned long long)));
-    if (!c->keep_count) FP_CUDA(c, cudaMemsetAsync(c->count_dev, 0, 2 * sizeof(unsigned long long), st));
+    // the sample count restarts with every call; the error flag stays up until it is read (fp_check)
+    if (!c->keep_count) FP_CUDA(c, cudaMemsetAsync(c->count_dev, 0, sizeof(unsigned long long), st));
     c->counted = c->opt_count != 0;
 
     if (!ids_tx.empty()) {
@@ -727,7 +777,7 @@ extern "C" fp_status fp_project(fp_ctx *c, const float *vol_dev, int n_proj, con
         FP_CUDA(c, cudaGetLastError());
         c->last_launches += 1;
     }
-    return FP_OK;
+    return leave_stream(c, st);
 }
 
 extern "C" fp_status fp_backproject(fp_ctx *c, const float *proj_dev, int n_proj, const double *geom, int nu, int nv,
@@ -738,10 +788,11 @@ extern "C" fp_status fp_backproject(fp_ctx *c, const float *proj_dev, int n_proj
     if (!vol_out_dev) return fail(c, FP_ERR_INVALID_ARG, "null pointer");
     cudaStream_t st = (cudaStream_t)stream;
     c->last_launches = 0;
-    c->last_stream = st;
     c->counted = false;
+    s = enter_stream(c, st);
+    if (s != FP_OK) return s;
     FP_CUDA(c, cudaMemsetAsync(vol_out_dev, 0, n_voxels(c) * sizeof(float), st));
-    if (n_proj == 0) return FP_OK;
+    if (n_proj == 0) return leave_stream(c, st);
     s = upload_geometry(c, n_proj, geom, nu, nv, false, st);
     if (s != FP_OK) return s;
     BackprojectParams B;
@@ -761,7 +812,7 @@ extern "C" fp_status fp_backproject(fp_ctx *c, const float *proj_dev, int n_proj
         fp_backproject_kernel<0><<<grid, kDirectThreads, 0, st>>>(B);
     FP_CUDA(c, cudaGetLastError());
     c->last_launches += 1;
-    return FP_OK;
+    return leave_stream(c, st);
 }
 
 extern "C" fp_status fp_ray_ranges(fp_ctx *c, int n_proj, const double *geom, int nu, int nv, int32_t *mfl_dev,
@@ -771,24 +822,36 @@ extern "C" fp_status fp_ray_ranges(fp_ctx *c, int n_proj, const double *geom, in
     if (s != FP_OK) return s;
     if (n_proj == 0) return FP_OK;
     cudaStream_t st = (cudaStream_t)stream;
+    s = enter_stream(c, st);
+    if (s != FP_OK) return s;
     s = upload_geometry(c, n_proj, geom, nu, nv, false, st);
     if (s != FP_OK) return s;
     dim3 grid((unsigned)((nu + 31) / 32), (unsigned)((nv + 7) / 8), (unsigned)n_proj);
     fp_ranges_kernel<<<grid, 256, 0, st>>>(c->G, c->proj_dev, nu, nv, mfl_dev);
     FP_CUDA(c, cudaGetLastError());
-    return FP_OK;
+    return leave_stream(c, st);
 }
 
 extern "C" fp_status fp_last_sample_count(fp_ctx *c, unsigned long long *n)
 {
     if (!c || !n) return FP_ERR_INVALID_ARG;
     *n = 0;
+    unsigned long long h[2];
+    fp_status s = read_counters(c, h);
+    if (s != FP_OK) return s;
+    if (h[1] != 0) return fail(c, FP_ERR_UNSUPPORTED, kPlanError);
     if (!c->counted || !c->count_dev) return fail(c, FP_ERR_INVALID_ARG, "no counted fp_project call to report");
-    FP_CUDA(c, cudaStreamSynchronize(c->last_stream));
-    unsigned long long h[2] = {0, 0};
-    FP_CUDA(c, cudaMemcpy(h, c->count_dev, sizeof h, cudaMemcpyDeviceToHost));
-    if (h[1] != 0) return fail(c, FP_ERR_CUDA, "internal error: a staging window or row tile of the aligned / TMA kernel did not fit (host plan too small)");
     *n = h[0];
+    return FP_OK;
+}
+
+extern "C" fp_status fp_check(fp_ctx *c)
+{
+    if (!c) return FP_ERR_INVALID_ARG;
+    unsigned long long h[2];
+    fp_status s = read_counters(c, h);
+    if (s != FP_OK) return s;
+    if (h[1] != 0) return fail(c, FP_ERR_UNSUPPORTED, kPlanError);
     return FP_OK;
 }
 
@@ -845,8 +908,9 @@ extern "C" fp_status fp_project_host(fp_ctx *c, const float *vol_host, int n_pro
     // synchronisation inside the loop; the shared geometry buffer is safe because all kernels are in one stream)
     cudaStream_t compute = c->hstream[0], copy = c->hstream[1];
     FP_CUDA(c, cudaMemcpyAsync(c->hvol_dev, vol_host, nvox * sizeof(float), cudaMemcpyHostToDevice, compute));
-    if (!c->count_dev) FP_CUDA(c, cudaMalloc(&c->count_dev, 2 * sizeof(unsigned long long)));
-    FP_CUDA(c, cudaMemsetAsync(c->count_dev, 0, 2 * sizeof(unsigned long long), compute));
+    s = enter_stream(c, compute);
+    if (s != FP_OK) return s;
+    FP_CUDA(c, cudaMemsetAsync(c->count_dev, 0, sizeof(unsigned long long), compute));
     // the layout copy (if any) is made once, then kept for all batches
     const int was_volatile = c->opt_volatile;
     int launches = 0;
@@ -882,5 +946,18 @@ extern "C" fp_status fp_project_host(fp_ctx *c, const float *vol_host, int n_pro
     c->last_launches = launches;
     c->last_stream = compute;
     c->counted = c->opt_count != 0;
+    // a window or row tile that did not fit (the host plan was too small): the call is repeated with the
+    // general-pose kernel, which has no such limit, instead of returning wrong numbers
+    unsigned long long h[2];
+    s = read_counters(c, h);
+    if (s != FP_OK) return s;
+    if (h[1] != 0 && c->opt_kernel != FP_KERNEL_DIRECT) {
+        const int was_kernel = c->opt_kernel;
+        c->opt_kernel = FP_KERNEL_DIRECT;
+        s = fp_project_host(c, vol_host, n_proj, geom, nu, nv, out_host);
+        c->opt_kernel = was_kernel;
+        return s;
+    }
+    if (h[1] != 0) return fail(c, FP_ERR_UNSUPPORTED, kPlanError);
     return FP_OK;
 }

@@ -59,8 +59,9 @@ struct __align__(16) AlLine {   // per staged line (column, slice of the batch)
 };
 
 struct __align__(16) AlBatch {  // per batch: the common z window of all its lines
-    double off;            // s_z - z0
+    double off;            // s_z - (z0 + zc): positions are taken relative to the window's centre
     int z0, nq;            // window origin (multiple of 4), float4 quads to stage
+    int zc, pad_;          // centre of the window relative to z0
 };
 
 struct __align__(16) AlShared {
@@ -70,10 +71,10 @@ struct __align__(16) AlShared {
     AlBatch batch[2];
     double s_z, rho_first, rho_last;
     int n_batches;
-    unsigned lines_bias;   // shared-window byte address of the staged lines minus (0x4B000000 << 2)
+    unsigned lines_bias;   // shared-window byte address of the staged lines minus (0x4B400000 << 2)
 };
 
-static_assert(sizeof(AlShared) % 16 == 0 && sizeof(AlLine) == 32 && sizeof(AlBatch) == 16, "shared layout");
+static_assert(sizeof(AlShared) % 16 == 0 && sizeof(AlLine) == 32 && sizeof(AlBatch) == 32, "shared layout");
 
 template <int W>
 constexpr size_t aligned_smem_bytes() { return sizeof(AlShared) + sizeof(float) * (size_t)kAlNL * W; }
@@ -149,7 +150,9 @@ __device__ __forceinline__ void al_batch_params(AlShared &S, const AlignedParams
     if (l == 0) {
         if (!winok) atomicOr(P.err_flag, 1u);
         AlBatch B;
-        B.off = winok ? S.s_z - (double)z0 : 4.0;
+        B.zc = winok ? need >> 1 : 0;
+        B.pad_ = 0;
+        B.off = winok ? S.s_z - (double)(z0 + B.zc) : 4.0;
         B.z0 = winok ? z0 : 0;
         B.nq = winok ? (need + 3) >> 2 : 0;
         S.batch[buf] = B;
@@ -232,7 +235,7 @@ fp_aligned_kernel(const __grid_constant__ AlignedParams P)
             S.s_z = s[2];
             S.rho_first = al_rho(g, P.G, row0, s[2]);
             S.rho_last = al_rho(g, P.G, min(row0 + kAlTV, P.nv) - 1, s[2]);
-            S.lines_bias = (unsigned)__cvta_generic_to_shared(lines) - (0x4B000000u << 2);
+            S.lines_bias = (unsigned)__cvta_generic_to_shared(lines) - (0x4B400000u << 2);
         }
     }
     __syncthreads();
@@ -295,8 +298,8 @@ fp_aligned_kernel(const __grid_constant__ AlignedParams P)
     const int nz = P.G.n[2];
     const int warp = tid >> 5, lane = tid & 31;
     constexpr int kWarps = kAlTV / 32;
-    const float2 kMagic2 = make_float2(8388608.0f, 8388608.0f);      // 2^23
-    const float2 kNegMagic2 = make_float2(-8388608.0f, -8388608.0f);
+    const float2 kMagic2 = make_float2(12582912.0f, 12582912.0f);    // 1.5 * 2^23 (positions may be negative)
+    const float2 kNegMagic2 = make_float2(-12582912.0f, -12582912.0f);
     const float2 kNegOne2 = make_float2(-1.0f, -1.0f);
 
     for (int b = 0; b < n_batches; ++b) {
@@ -335,17 +338,19 @@ fp_aligned_kernel(const __grid_constant__ AlignedParams P)
         if (tid < kAlNL && b + 1 < n_batches) al_batch_params<INTERP, W, true>(S, P, buf ^ 1, b + 1, tid);
         __syncthreads();
         // ---------------- phase B
+        // positions relative to the CENTRE of the window (|p| <= W / 2: one more bit of fp32 precision)
+        const unsigned bias_b = lines_bias + (unsigned)(B.zc * 4);
 #pragma unroll
         for (int c = 0; c < kAlTU; ++c) {
             const float a = (float)fma(S.t0[buf][c], rho, B.off);
 #pragma unroll
             for (int s = 0; s < kAlSB; s += 2) {
                 const float2 p = __ffma2_rn(make_float2((float)s, (float)(s + 1)), make_float2(dz[c], dz[c]), make_float2(a, a));
-                const float2 x = __fadd2_rd(p, kMagic2);                  // bits = 0x4B000000 + floor(p)
+                const float2 x = __fadd2_rd(p, kMagic2);                  // bits = 0x4B400000 + floor(p)
                 const float2 f = __fadd2_rn(x, kNegMagic2);
                 const float2 d = __ffma2_rn(f, kNegOne2, p);              // p - floor(p)
-                const unsigned a0 = (__float_as_uint(x.x) << 2) + lines_bias + (unsigned)((c * kAlSB + s) * W * 4);
-                const unsigned a1 = (__float_as_uint(x.y) << 2) + lines_bias + (unsigned)((c * kAlSB + s + 1) * W * 4);
+                const unsigned a0 = (__float_as_uint(x.x) << 2) + bias_b + (unsigned)((c * kAlSB + s) * W * 4);
+                const unsigned a1 = (__float_as_uint(x.y) << 2) + bias_b + (unsigned)((c * kAlSB + s + 1) * W * 4);
                 const float2 v0 = make_float2(al_lds(a0), al_lds(a1));
                 const float2 v1 = make_float2(al_lds(a0 + 4u), al_lds(a1 + 4u));
                 const float2 wz = make_float2(ceil_weight<INTERP>(d.x), ceil_weight<INTERP>(d.y));

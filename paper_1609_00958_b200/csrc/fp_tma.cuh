@@ -37,7 +37,8 @@ constexpr int kTmWMin = 160, kTmWStep = 32;
 constexpr int kTmNR = 12;                // most volume rows per tile (largest box)
 constexpr int kTmMaps = 5;               // tensor maps per pass: boxes of 4, 6, 8, 10, 12 rows
 constexpr int kTmStageFloats = kTmNR * kTmW;
-constexpr unsigned kTmTileBytes = kTmSB * kTmStageFloats * 4u;   // 48 KB of tiles; two zero rows follow
+constexpr unsigned kTmTileBytes = kTmSB * kTmStageFloats * 4u;   // 48 KB of tiles; the zero region follows
+constexpr int kTmZeroFloats = 3 * kTmW;  // zeros for columns without a sample: window positions -128 .. 128, rows j and j + 1
 
 struct __align__(64) TmaParams {
     CUtensorMap map[2][kTmWBoxes][kTmMaps];   // [pass = driving axis x / y][box width][box of 4, 6, 8, 10 or 12 rows]
@@ -220,9 +221,11 @@ __device__ __forceinline__ void tm_produce_batch(TmShared &S, const TmaParams &P
     if (!winok && lane == 0) atomicOr(P.err_flag, 1u);
     const int bp = gb & 1;
     if (s == 0) S.t0[bp][c] = winok ? __dmul_rn(__dsub_rn((double)i0, S.s_m), C.inv_rm) : 0.0;
-    // a window that does not fit is never sampled out of bounds: park every row at p = 4
+    // positions are taken relative to the centre of the window (|p| <= 128: one more bit of fp32 precision than
+    // relative to its start); a window that does not fit is never sampled out of bounds: every row is parked at p = 4
+    const int zc = winok ? (need >> 1) : 0;
     if (lane == 0) {
-        S.off[bp] = winok ? S.s[2] - (double)z0 : 4.0;
+        S.off[bp] = winok ? S.s[2] - (double)(z0 + zc) : 4.0;
         S.pitch[bp] = (unsigned)(pitch * 4);
     }
     const bool use = fits && winok;
@@ -239,8 +242,11 @@ __device__ __forceinline__ void tm_produce_batch(TmShared &S, const TmaParams &P
         const unsigned bytes = (info_s & 1) ? (unsigned)((4 + 2 * mi_s) * pitch * 4) : 0u;
         if (gb > 0) tm_mbar_wait(&S.empty[ss], (gb - 1) & 1);
         const unsigned phys = (unsigned)(ss * kTmStageFloats * 4);
-        // a column without a sample on this slice reads the two zero rows behind the tiles
-        if (s == ss) S.stage_col[ss][c] = make_uint2(use ? phys + row_off : kTmTileBytes, wbits);
+        // published: the shared-window address of the word at window position p = 0 of the column's lower row, minus
+        // (0x4B400000 << 2) -- the consumers add (bits of p + 1.5 * 2^23) << 2.  A column without a sample on this slice
+        // reads the zero region behind the tiles (from its position 128 on: p may be negative).
+        const unsigned addr0 = tiles_smem - (0x4B400000u << 2) + (use ? phys + row_off + (unsigned)(zc * 4) : kTmTileBytes + (unsigned)(kTmW / 2) * 4u);
+        if (s == ss) S.stage_col[ss][c] = make_uint2(addr0, wbits);
         __syncwarp();
         if (lane == 0) {
             if (bytes) {
@@ -277,8 +283,8 @@ __global__ void __launch_bounds__(kTmThreads, 4)
 fp_tma_kernel(const __grid_constant__ TmaParams P)
 {
     extern __shared__ __align__(128) unsigned char tm_smem_raw[];
-    float *tiles = reinterpret_cast<float *>(tm_smem_raw);                   // kTmSB stages, then two zero rows; 128-byte aligned
-    TmShared &S = *reinterpret_cast<TmShared *>(tm_smem_raw + kTmTileBytes + sizeof(float) * 2 * kTmW);
+    float *tiles = reinterpret_cast<float *>(tm_smem_raw);                   // kTmSB stages, then the zero region; 128-byte aligned
+    TmShared &S = *reinterpret_cast<TmShared *>(tm_smem_raw + kTmTileBytes + sizeof(float) * kTmZeroFloats);
 
     const int tid = threadIdx.x, lane = tid & 31;
     // the shuffle tells the compiler that the warp index (and with it the role) is warp-uniform
@@ -321,7 +327,7 @@ fp_tma_kernel(const __grid_constant__ TmaParams P)
             asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
         }
     }
-    for (int k = tid; k < 2 * kTmW; k += blockDim.x) tiles[kTmSB * kTmStageFloats + k] = 0.0f;
+    for (int k = tid; k < kTmZeroFloats; k += blockDim.x) tiles[kTmSB * kTmStageFloats + k] = 0.0f;
     __syncthreads();
 
     // Two roles, one code region each (so that no role carries another role's registers); every warp
@@ -340,7 +346,6 @@ fp_tma_kernel(const __grid_constant__ TmaParams P)
         }
     } else {
         const double rho0 = al_rho(g, P.G, iv0, S.s[2]), rho1 = al_rho(g, P.G, iv1, S.s[2]);
-        const unsigned tile_bias = tm_smem(tiles) - (0x4B400000u << 2);
         const float2 kMagic2 = make_float2(12582912.0f, 12582912.0f);    // 1.5 * 2^23
         const float2 kNegMagic2 = make_float2(-12582912.0f, -12582912.0f);
         const float2 kNegOne2 = make_float2(-1.0f, -1.0f);
@@ -362,6 +367,8 @@ fp_tma_kernel(const __grid_constant__ TmaParams P)
             for (int b = 0; b < n_batches; ++b, ++gb) {
                 const unsigned par = gb & 1;
                 tm_mbar_wait(&S.full[0], par);
+                // Eq. 6 for z per (column, row), relative to the CENTRE of the batch's window: p = a + s dz
+                // with |p| <= 128, i.e. fp32 positions good to 4e-6 voxel
                 float2 a[kTmTU];
                 unsigned pitchB;
                 {
@@ -387,8 +394,8 @@ fp_tma_kernel(const __grid_constant__ TmaParams P)
                         const float2 x = __fadd2_rd(p, kMagic2);                  // bits = 0x4B400000 + floor(p)
                         const float2 f = __fadd2_rn(x, kNegMagic2);
                         const float2 d = __ffma2_rn(f, kNegOne2, p);              // p - floor(p)
-                        const unsigned rb = tile_bias + pc.x;
-                        const unsigned a0 = (__float_as_uint(x.x) << 2) + rb, a1 = (__float_as_uint(x.y) << 2) + rb;
+                        // pc.x = shared-window address of word 0 of the column's lower row minus (0x4B400000 << 2)
+                        const unsigned a0 = (__float_as_uint(x.x) << 2) + pc.x, a1 = (__float_as_uint(x.y) << 2) + pc.x;
                         const float2 v00 = make_float2(al_lds(a0), al_lds(a1));
                         const float2 v01 = make_float2(al_lds(a0 + 4u), al_lds(a1 + 4u));
                         const unsigned b0 = a0 + pitchB, b1 = a1 + pitchB;        // row j + 1
@@ -435,6 +442,6 @@ fp_tma_kernel(const __grid_constant__ TmaParams P)
     if (P.sample_count) block_count_samples(P.sample_count, n_samples);
 }
 
-constexpr size_t tma_smem_bytes() { return kTmTileBytes + sizeof(float) * 2 * kTmW + sizeof(TmShared); }
+constexpr size_t tma_smem_bytes() { return kTmTileBytes + sizeof(float) * kTmZeroFloats + sizeof(TmShared); }
 
 }  // namespace fpk

@@ -18,14 +18,15 @@ LIB_PATH = os.path.join(_HERE, "libfp.so")
 FP_OK = 0
 STATUS = {0: "FP_OK", 1: "FP_ERR_INVALID_ARG", 2: "FP_ERR_CUDA", 3: "FP_ERR_OOM", 4: "FP_ERR_UNSUPPORTED"}
 
-OPT_KERNEL, OPT_VOLATILE, OPT_INTERP, OPT_PERMUTED_COPY, OPT_COUNT_SAMPLES, OPT_FOV_CYLINDER = 1, 2, 3, 4, 5, 6
+OPT_KERNEL, OPT_VOLATILE, OPT_INTERP, OPT_PERMUTED_COPY, OPT_COUNT_SAMPLES, OPT_FOV_CYLINDER, OPT_GROUP = 1, 2, 3, 4, 5, 6, 7
+OPT_TEST_FORCE_TMA = 100
 KERNEL_AUTO, KERNEL_DIRECT, KERNEL_ALIGNED, KERNEL_TMA, KERNEL_TEX, KERNEL_HWLIN = 0, 1, 2, 3, 4, 5
 INTERP_LINEAR, INTERP_SPLINE = 0, 1
 
 # every symbol include/fp.h declares (tests check the library exports all of them)
 SYMBOLS = ["fp_create", "fp_destroy", "fp_set_option", "fp_get_option", "fp_prepare", "fp_project",
-           "fp_project_host", "fp_backproject", "fp_ray_ranges", "fp_plan", "fp_last_sample_count", "fp_last_launch_count",
-           "fp_status_string", "fp_last_error", "fp_version"]
+           "fp_project_host", "fp_backproject", "fp_ray_ranges", "fp_plan", "fp_check", "fp_last_sample_count",
+           "fp_last_launch_count", "fp_status_string", "fp_last_error", "fp_version"]
 
 
 class FpError(RuntimeError):
@@ -65,7 +66,8 @@ def load(build_if_missing: bool = True):
     L.fp_plan.argtypes = [vp, dp, i, i, ctypes.POINTER(i), ctypes.POINTER(i), ctypes.POINTER(i)]
     L.fp_last_sample_count.argtypes = [vp, ctypes.POINTER(ctypes.c_ulonglong)]
     L.fp_last_launch_count.argtypes = [vp, ctypes.POINTER(i)]
-    for name in ("fp_create", "fp_destroy", "fp_set_option", "fp_get_option", "fp_prepare", "fp_project",
+    L.fp_check.argtypes = [vp]
+    for name in ("fp_create", "fp_destroy", "fp_set_option", "fp_get_option", "fp_prepare", "fp_project", "fp_check",
                  "fp_project_host", "fp_backproject", "fp_ray_ranges", "fp_plan", "fp_last_sample_count", "fp_last_launch_count"):
         getattr(L, name).restype = i
     L.fp_status_string.argtypes = [i]
@@ -217,6 +219,10 @@ class Projector:
         self._check(self._L.fp_plan(self._h, g.ctypes.data_as(ctypes.POINTER(ctypes.c_double)), int(nu), int(nv),
                                     ctypes.byref(k), ctypes.byref(w), ctypes.byref(z)))
         return k.value, w.value, bool(z.value)
+
+    def check(self) -> None:
+        """fp_check: raises FpError if a kernel since the last check found the host plan too small."""
+        self._check(self._L.fp_check(self._h))
 
     def last_sample_count(self) -> int:
         n = ctypes.c_ulonglong()

@@ -546,3 +546,58 @@ def test_backprojection_adjoint_identity_and_linearity(oracle):
     bp = oracle.backproject(np.abs(y1), shape, delta, origin, geom)
     assert bp.min() >= 0.0
     assert abs(float((a1 * np.abs(y1)).sum()) - float(bp.sum())) <= 1e-10 * float(bp.sum())
+
+
+# ---------------------------------------------------------------- given-axis rays (reading #8) and voxel-list transpose
+
+def test_given_axis_equals_chosen_axis_and_axis_swap_on_ties(oracle):
+    """jo_ray_grid_axis is pinned without calling itself twice: (1) with the axis Eq. 2 chooses it returns the
+    bits of the pinned jo_ray_grid; (2) on an EXACT tie |r_x| = |r_y| the sum along y equals the chosen-axis sum
+    of the problem with the x and y axes swapped (there Eq. 2's lowest-index rule picks the old y)."""
+    rng = np.random.default_rng(81)
+    vol = rand_vol(rng, (7, 6, 5))
+    geom = np.array([[-30.0, 2.0, 1.0, 40.0, -8.0, -6.0, 0.0, 1.1, 0.0, 0.0, 0.0, 1.3]])
+    ids = np.array([(0, iv, iu) for iv in range(10) for iu in range(14)], dtype=np.int32)
+    origin, delta = (-3.1, -2.4, -2.2), 0.9
+    val, mfl, pl, _ = oracle.project_rays(vol, delta, origin, geom, ids)
+    val2, mfl2, pl2 = oracle.project_rays_axis(vol, delta, origin, geom, ids, mfl[:, 0])
+    assert np.array_equal(val, val2) and np.array_equal(mfl, mfl2) and np.array_equal(pl, pl2)
+    assert len(np.unique(mfl[:, 0])) >= 1 and np.abs(val).max() > 0.1
+    # exact ties, grid coordinates: r = (a, +-a, c) with |c| < |a|
+    n_checked = 0
+    for _ in range(40):
+        s = np.array([rng.uniform(-9, -4), rng.uniform(-3, 9), rng.uniform(-2, 7)])
+        a = float(rng.integers(12, 24))
+        sign = 1.0 if rng.random() < 0.5 else -1.0
+        d = s + np.array([a, sign * a, rng.uniform(-0.4, 0.4) * a])
+        if abs(d[0] - s[0]) != abs(d[1] - s[1]):
+            continue                                                      # rounding broke the tie
+        assert oracle.ray_grid(vol, s, d)["m"] == 0                        # Eq. 2, reading #8
+        got = oracle.ray_grid_axis(vol, s, d, 1)
+        pv = np.ascontiguousarray(np.transpose(vol, (1, 0, 2)))
+        ref = oracle.ray_grid(pv, s[[1, 0, 2]], d[[1, 0, 2]])
+        assert ref["m"] == 0
+        assert abs(got["value"] - ref["value"]) <= 1e-13 * (1 + abs(ref["value"]))        # tap order differs
+        assert (got["i_first"], got["i_last"]) == (ref["i_first"], ref["i_last"])
+        n_checked += ref["i_last"] >= ref["i_first"]
+    assert n_checked >= 10
+
+
+@pytest.mark.parametrize("kernel", [0, 1])
+def test_voxel_list_backprojection_equals_full_backprojection(oracle, kernel):
+    """jo_backproject_voxels (the transpose by its definition, one hat product per ray and voxel, rays limited
+    to a detector window) against the pinned jo_backproject on every voxel of small grids with all three
+    driving axes -- which also shows that the window is wide enough for these magnifications."""
+    rng = np.random.default_rng(82)
+    shape, delta, nu, nv = (9, 7, 8), 0.8, 15, 13
+    origin = tuple(-(n - 1) / 2.0 * delta + 0.05 * k for k, n in enumerate(shape))
+    geom = _bp_poses(shape, delta, nu, nv)
+    y = rng.uniform(-1.0, 2.0, size=(len(geom), nv, nu))
+    full = oracle.backproject(y, shape, delta, origin, geom, kernel=kernel)
+    vox = np.array(list(itertools.product(*[range(n) for n in shape])), dtype=np.int32)
+    got = oracle.backproject_voxels(y, shape, delta, origin, geom, vox, halfwin=4, kernel=kernel, threads=2)
+    assert np.abs(full).max() > 0.1
+    assert np.allclose(got, full.reshape(-1), rtol=0, atol=1e-12 * np.abs(full).max())
+    # a window that is too narrow must show up as a difference (the check above is not vacuous)
+    narrow = oracle.backproject_voxels(y, shape, delta, origin, geom, vox, halfwin=0, kernel=kernel)
+    assert np.abs(narrow - full.reshape(-1)).max() > 1e-3

@@ -6,7 +6,7 @@ import math
 import numpy as np
 import pytest
 
-from parity_util import assert_parity
+from parity_util import assert_parity, make_recompute
 
 pytestmark = pytest.mark.gpu
 
@@ -54,7 +54,8 @@ def compare_full(torch, fp, oracle, vol_np, delta, origin, geom, nu, nv, options
     out, mfl, n = run_gpu(torch, fp, vol_np, delta, origin, geom, nu, nv, options)
     ids = all_ids(geom.shape[0], nv, nu)
     ov, om, pl, mg = oracle.project_rays(vol_np, delta, origin, geom, ids, kernel=kernel, threads=oracle.host_cores())
-    worst = assert_parity(out.ravel(), mfl.reshape(-1, 3), ov, om, pl, mg, float(np.abs(vol_np).max()), what)
+    worst = assert_parity(out.ravel(), mfl.reshape(-1, 3), ov, om, pl, mg, float(np.abs(vol_np).max()), what,
+                          recompute=make_recompute(oracle, vol_np, delta, origin, geom, ids, kernel))
     assert n == int(np.maximum(om[:, 2] - om[:, 1] + 1, 0).sum()), "sample count"
     return worst, out, om
 
@@ -83,7 +84,8 @@ def test_c2_128_cube_full_orbit(torch, fp, synth, oracle):
     ov, om, pl, mg = oracle.project_rays(vol, cfg.voxel_size, cfg.origin, geom, ids, threads=oracle.host_cores())
     g = out[ids[:, 0], ids[:, 1], ids[:, 2]]
     gm = mfl[ids[:, 0], ids[:, 1], ids[:, 2]]
-    assert assert_parity(g, gm, ov, om, pl, mg, float(np.abs(vol).max()), "C2") < 1.0
+    assert assert_parity(g, gm, ov, om, pl, mg, float(np.abs(vol).max()), "C2",
+                         recompute=make_recompute(oracle, vol, cfg.voxel_size, cfg.origin, geom, ids)) < 1.0
     assert n == int(np.maximum(mfl[..., 2] - mfl[..., 1] + 1, 0).sum())
 
 
@@ -103,7 +105,7 @@ def test_c1_and_c2_through_the_direct_kernel(torch, fp, synth, oracle):
     assert worst < 1.0
 
 
-def _big_config_subset(torch, fp, synth, oracle, name, projs, n_random, batch=None):
+def _big_config_subset(torch, fp, synth, oracle, name, projs, n_random, batch=None, options=()):
     """Full-size volume on the device, the launch configuration bench.py times (whole batches
     through fp_project), compared on sampled rays the oracle computes one by one."""
     cfg = synth.CONFIGS[name]
@@ -112,6 +114,8 @@ def _big_config_subset(torch, fp, synth, oracle, name, projs, n_random, batch=No
     geom = synth.make_geometry(cfg)
     sub = geom[projs]
     with fp.Projector(*cfg.n, cfg.voxel_size, cfg.origin) as P:
+        for k, v in options:
+            P.set_option(k, v)
         out = P.project(vol_t, sub, cfg.nu, cfg.nv)
         mfl = P.ray_ranges(sub, cfg.nu, cfg.nv)
         torch.cuda.synchronize()
@@ -128,7 +132,8 @@ def _big_config_subset(torch, fp, synth, oracle, name, projs, n_random, batch=No
     ov, om, pl, mg = oracle.project_rays(vol, cfg.voxel_size, cfg.origin, sub, ids, threads=oracle.host_cores())
     g = out[ids[:, 0], ids[:, 1], ids[:, 2]]
     gm = mfl[ids[:, 0], ids[:, 1], ids[:, 2]]
-    worst = assert_parity(g, gm, ov, om, pl, mg, float(np.abs(vol).max()), name)
+    worst = assert_parity(g, gm, ov, om, pl, mg, float(np.abs(vol).max()), name,
+                          recompute=make_recompute(oracle, vol, cfg.voxel_size, cfg.origin, sub, ids))
     assert n == int(np.maximum(mfl[..., 2] - mfl[..., 1] + 1, 0).sum())
     return worst, om
 
@@ -148,6 +153,15 @@ def test_c4_wide_cone_general_poses_sampled(torch, fp, synth, oracle):
 def test_c5_large_volume_sampled(torch, fp, synth, oracle):
     worst, om = _big_config_subset(torch, fp, synth, oracle, "C5", [0, 89, 90, 91, 400, 719], 40000)
     assert worst < 1.0
+
+
+def test_p1_paper_shaped_sampled(torch, fp, synth, oracle):
+    """The paper-shaped workload at full size (512^3 cylinder -> 512^2, 10 degree cone, grid matched by Eq. 17;
+    PAPER.md:312-314, :326) with FP_OPT_FOV_CYLINDER, default plan (the 384-voxel instantiation of
+    fp_aligned_kernel with the circle clip), poses around the driving-axis switch included."""
+    worst, om = _big_config_subset(torch, fp, synth, oracle, "P1", [0, 44, 45, 46, 90, 135, 201, 359], 60000,
+                                   options=[(fp.OPT_FOV_CYLINDER, 1)])
+    assert worst < 1.0 and set(np.unique(om[:, 0])) == {0, 1}
 
 
 # ----------------------------------------------------------------------------- edge cases
@@ -500,6 +514,38 @@ def test_backprojection_c1_parity_and_adjoint_identity_at_c3_size(torch, fp, syn
     assert abs(lhs - rhs) <= 2e-5 * abs(lhs), (lhs, rhs)
 
 
+def test_backprojection_c3_size_sampled_voxels(torch, fp, synth, oracle):
+    """Element by element at full size: fp_backproject on the 512^3 grid of C3 (four poses, both driving axes),
+    compared on 2^18 seeded voxels plus the volume's corners and centre,
+    with (A^T y)[v] computed voxel by voxel from the definition of the transpose (oracle.backproject_voxels).
+    Tolerance as in bp_tolerance, with max_v (A^T 1) taken over the sampled voxels only (never larger)."""
+    cfg = synth.CONFIGS["C3"]
+    geom = synth.make_geometry(cfg)[[3, 47, 200, 311]]
+    gen = torch.Generator(device="cuda").manual_seed(6)
+    yy = torch.rand((len(geom), cfg.nv, cfg.nu), device="cuda", generator=gen) * 2.0 - 0.5
+    with fp.Projector(*cfg.n, cfg.voxel_size, cfg.origin) as P:
+        aty = P.backproject(yy, geom, cfg.nu, cfg.nv)
+        torch.cuda.synchronize()
+    rng = np.random.default_rng(cfg.seed + 99)
+    nx, ny, nz = cfg.n
+    vox = np.stack([rng.integers(0, nx, 1 << 18), rng.integers(0, ny, 1 << 18), rng.integers(0, nz, 1 << 18)], axis=1)
+    special = [(0, 0, 0), (nx - 1, ny - 1, nz - 1), (nx - 1, 0, 0), (0, ny - 1, nz - 1), (nx // 2, ny // 2, nz // 2),
+               (nx - 1, ny // 2, 3), (nx // 2 + 1, 0, 0)]
+    vox = np.concatenate([vox, np.array(special)]).astype(np.int32)
+    idx = torch.from_numpy(vox.astype(np.int64)).cuda()
+    g = aty[idx[:, 0], idx[:, 1], idx[:, 2]].cpu().numpy().astype(np.float64)
+    y = yy.cpu().numpy().astype(np.float64)
+    th = oracle.host_cores()
+    # the hat footprint of a voxel is +-1 voxel = +-(SDD / (SID - half diagonal)) = +-2.4 pixels here
+    ref = oracle.backproject_voxels(y, cfg.n, cfg.voxel_size, cfg.origin, geom, vox, halfwin=4, threads=th)
+    absy = oracle.backproject_voxels(np.abs(y), cfg.n, cfg.voxel_size, cfg.origin, geom, vox, halfwin=4, threads=th)
+    wsum = oracle.backproject_voxels(np.ones_like(y), cfg.n, cfg.voxel_size, cfg.origin, geom, vox, halfwin=4, threads=th)
+    tol = 2e-5 * absy + 1e-6 * float(wsum.max()) * float(np.abs(y).max())
+    err = np.abs(g - ref)
+    assert np.abs(ref).max() > 1.0 and (ref != 0).mean() > 0.5
+    assert np.all(err <= tol), (float(np.max(err / np.maximum(tol, 1e-300))), vox[int(np.argmax(err - tol))])
+
+
 def test_tma_kernel_follows_the_volume_pointer_and_contents(torch, fp, oracle):
     """The tensor maps of the TMA-fed kernel are cached per volume pointer: a second volume at another address
     and new contents at the same address must both be projected from the data as it is at call time."""
@@ -575,3 +621,133 @@ def test_cylinder_field_of_view_option(torch, fp, oracle, kernel_opt):
     ids = all_ids(len(geom), nv, nu)
     ov, om, pl, mg = oracle.project_rays(vol, delta, origin, geom, ids, threads=oracle.host_cores())
     assert assert_parity(cyl.ravel(), mfl.reshape(-1, 3), ov, om, pl, mg, float(np.abs(vol).max())) < 1.0
+
+
+# ----------------------------------------------------------------------------- host plan against the kernels' own checks
+
+def aligned_pose2(theta, sid, sdd, nu, nv, pitch_u, pitch_v, src_z=0.0, det_shift=(0.0, 0.0), flip_u=False, flip_v=False):
+    """aligned_pose with separate pixel pitches along u and v."""
+    c, s = math.cos(theta), math.sin(theta)
+    S = np.array([sid * c, sid * s, src_z])
+    C = S - sdd * np.array([c, s, 0.0])
+    U = pitch_u * np.array([-s, c, 0.0]) * (-1.0 if flip_u else 1.0)
+    V = pitch_v * np.array([0.0, 0.0, 1.0]) * (-1.0 if flip_v else 1.0)
+    O = C - ((nu - 1) / 2 + det_shift[0]) * U - ((nv - 1) / 2 + det_shift[1]) * V
+    return np.concatenate([S, O, U, V])
+
+
+def test_plan_overflow_is_reported_and_project_host_recovers(torch, fp, oracle):
+    """A pose whose tiles do not fit fp_tma_kernel, sent there by the test hook: the kernel's bound check raises
+    the flag, fp_check / fp_last_sample_count return FP_ERR_UNSUPPORTED (once: the read clears it), and
+    fp_project_host repeats the call with the general-pose kernel and returns the right projections."""
+    rng = np.random.default_rng(910)
+    shape = (40, 36, 64)
+    vol = rng.uniform(0.0, 1.0, size=shape).astype(np.float32)
+    delta = 1.0
+    origin = tuple(-(n - 1) / 2.0 * delta for n in shape)
+    nu, nv = 16, 64
+    # wide pixels along u: the eight columns of a block fan out over more than the 12 volume rows a tile holds
+    geom = np.stack([aligned_pose2(0.6, 60.0, 120.0, nu, nv, 3.0, 1.0), aligned_pose2(0.75, 60.0, 120.0, nu, nv, 3.0, 1.0)])
+    with fp.Projector(*shape, delta, origin) as P:
+        assert all(P.plan(g, nu, nv)[0] == fp.KERNEL_ALIGNED for g in geom)
+        vt = torch.from_numpy(vol).cuda()
+        P.project(vt, geom, nu, nv)
+        P.check()                                            # the default plan: nothing to report
+        P.set_option(fp.OPT_TEST_FORCE_TMA, 1)
+        P.project(vt, geom, nu, nv)
+        with pytest.raises(fp.FpError) as e:
+            P.check()
+        assert e.value.status == 4                           # FP_ERR_UNSUPPORTED
+        P.check()                                            # cleared by the read
+        P.set_option(fp.OPT_COUNT_SAMPLES, 0)
+        P.project(vt, geom, nu, nv)
+        with pytest.raises(fp.FpError) as e:
+            P.last_sample_count()                            # reported even when the call did not count
+        assert e.value.status == 4
+        # the end-to-end entry point notices and repeats the call with the direct kernel
+        out = P.project_host(vol, geom, nu, nv)
+        P.check()
+    ids = all_ids(len(geom), nv, nu)
+    ov, om, pl, mg = oracle.project_rays(vol, delta, origin, geom, ids, threads=oracle.host_cores())
+    tol = 2e-5 * np.abs(ov) + 1e-6 * pl * float(np.abs(vol).max())
+    assert np.all(np.abs(out.numpy().ravel().astype(np.float64) - ov) <= tol)
+
+
+def phantom_like_volume(rng, shape):
+    """The BASELINE recipe in miniature: a few overlapping random boxes with values in [0, 1] plus Gaussian noise
+    of sigma 0.01 (flat regions, unit edges) -- unlike the uniform-noise volumes of the edge-case tests, whose
+    voxel-to-voxel jumps are as large as max|voxel| everywhere."""
+    v = rng.normal(0.0, 0.01, size=shape)
+    for _ in range(6):
+        lo = [int(rng.integers(0, n - 2)) for n in shape]
+        hi = [int(rng.integers(l + 2, n + 1)) for l, n in zip(lo, shape)]
+        v[lo[0]:hi[0], lo[1]:hi[1], lo[2]:hi[2]] += rng.uniform(0.0, 1.0)
+    return v.astype(np.float32)
+
+
+def test_random_aligned_poses_never_trip_the_kernels_bound_checks(torch, fp, oracle):
+    """2400 random poses of the aligned class (source distance, magnification, pixel pitches, detector size and
+    shifts, source height, both flips, volume shapes) through the default plan: the kernels' own window / row-tile
+    checks must never fire (fp_check), every pose the plan gives to the TMA or aligned kernel included, and a
+    sample of them is compared with the oracle ray by ray."""
+    rng = np.random.default_rng(911)
+    shapes = [(48, 40, 32), (33, 57, 64), (64, 64, 96), (20, 90, 44)]
+    kernels_seen = set()
+    n_checked = 0
+    for si, shape in enumerate(shapes):
+        vol = phantom_like_volume(rng, shape)
+        delta = float(rng.uniform(0.4, 1.6))
+        origin = tuple(-(n - 1) / 2.0 * delta + rng.uniform(-0.3, 0.3) for n in shape)
+        vt = torch.from_numpy(vol).cuda()
+        half = 0.5 * delta * math.hypot(shape[0], shape[1])
+        with fp.Projector(*shape, delta, origin) as P:
+            for q in range(600):
+                nu, nv = int(rng.integers(1, 70)), int(rng.integers(1, 600))
+                sid = half * float(rng.uniform(1.05, 12.0))
+                sdd = sid * float(rng.uniform(1.05, 3.0))
+                zext = shape[2] * delta
+                pitch_v = zext * (sdd / sid) * float(rng.uniform(0.3, 2.5)) / nv
+                pitch_u = 2 * half * (sdd / sid) * float(rng.uniform(0.2, 1.5)) / max(nu, 8)
+                g = aligned_pose2(float(rng.uniform(0, 2 * math.pi)), sid, sdd, nu, nv, pitch_u, pitch_v,
+                                  src_z=float(rng.uniform(-0.6, 0.6)) * zext,
+                                  det_shift=(float(rng.uniform(-0.3, 0.3)) * nu, float(rng.uniform(-0.3, 0.3)) * nv),
+                                  flip_u=bool(rng.integers(0, 2)), flip_v=bool(rng.integers(0, 2)))
+                kernels_seen.add(P.plan(g, nu, nv)[0])
+                out = P.project(vt, g[None], nu, nv)
+                if q % 40 == 0:
+                    P.check()
+                    ids = all_ids(1, nv, nu)
+                    ov, om, pl, mg = oracle.project_rays(vol, delta, origin, g[None], ids, threads=oracle.host_cores())
+                    gm = P.ray_ranges(g[None], nu, nv).cpu().numpy().reshape(-1, 3)
+                    worst = assert_parity(out.cpu().numpy().ravel(), gm, ov, om, pl, mg, float(np.abs(vol).max()),
+                                          "random aligned pose %d/%d" % (si, q),
+                                          recompute=make_recompute(oracle, vol, delta, origin, g[None], ids))
+                    assert worst < 1.0
+                    n_checked += 1
+            P.check()
+    assert fp.KERNEL_TMA in kernels_seen and fp.KERNEL_ALIGNED in kernels_seen
+    assert n_checked >= 60
+
+
+def test_output_pointer_that_is_only_four_byte_aligned(torch, fp, oracle):
+    """out_dev one float past a 16-byte boundary: the aligned / TMA kernels must fall back to scalar stores
+    (a float4 store there would fault)."""
+    rng = np.random.default_rng(912)
+    shape = (24, 20, 32)
+    vol = rng.uniform(0.0, 1.0, size=shape).astype(np.float32)
+    delta, nu, nv = 1.0, 16, 40
+    origin = tuple(-(n - 1) / 2.0 * delta for n in shape)
+    geom = np.stack([aligned_pose(t, 80.0, 160.0, nu, nv, 1.5) for t in (0.1, 0.8, 2.0)])
+    vt = torch.from_numpy(vol).cuda()
+    buf = torch.zeros(len(geom) * nv * nu + 1, device="cuda", dtype=torch.float32)
+    view = buf[1:].view(len(geom), nv, nu)
+    assert view.data_ptr() % 16 == 4
+    with fp.Projector(*shape, delta, origin) as P:
+        for kern in (fp.KERNEL_AUTO, fp.KERNEL_ALIGNED):
+            P.set_option(fp.OPT_KERNEL, kern)
+            ref = P.project(vt, geom, nu, nv)
+            got = P.project(vt, geom, nu, nv, out=view)
+            torch.cuda.synchronize()
+            assert torch.equal(ref, got)
+            P.check()
+    assert float(buf[0]) == 0.0
