@@ -14,6 +14,7 @@ from __future__ import annotations
 
 import argparse
 import json
+import math
 import os
 import statistics
 import subprocess
@@ -31,9 +32,27 @@ METRIC = "512^3 cone-beam projections/s"
 UNIT = "projections/s"
 TAP_BYTES = 16           # 4 taps x 4 B per sample: the paper's "memory access rate"
 FALLBACK_HBM_GBS = 6650.0
-# dram__bytes_read.sum + dram__bytes_write.sum of one launch, from the committed ncu --set full captures
-# (profiles/r1_02_aligned_kernel_c3.md, profiles/r1_03_tma_kernel_c3.md); None where no capture exists
-NCU_TRAFFIC_BYTES = {("C3", "fp_aligned_kernel"): 201.51e9, ("C3", "fp_tma_kernel"): 223.54e9}
+TRAFFIC_JSON = os.path.join(ROOT, "profiles", "traffic.json")
+
+
+def csrc_sha():
+    """Hash of the library's sources: profiles/traffic.json records it with every ncu capture, and a capture is
+    quoted only while the sources it was taken from are the ones being timed."""
+    from paper_1609_00958_b200.ncu_traffic import csrc_sha as f
+    return f()
+
+
+def captured_traffic(config, kernel, interp):
+    """(entry, stale) for this config / kernel from profiles/traffic.json (written by
+    python -m paper_1609_00958_b200.ncu_traffic from an ncu --set full capture)."""
+    try:
+        db = json.load(open(TRAFFIC_JSON))
+    except Exception:
+        return None, False
+    e = db.get("%s/%s/%s" % (config, kernel, interp))
+    if e is None:
+        return None, False
+    return e, e.get("csrc_sha") != csrc_sha()
 
 
 def measured_peaks():
@@ -99,13 +118,13 @@ class ClockSampler:
         return out
 
 
-def oracle_sample(cfg, geom, vol_np, max_seconds=20.0, kernel=0):
-    """Time the oracle, as it stands, on a bounded sample of the workload: whole detector rows of
-    projection 0 and of the projection at 1/8 of the orbit (both driving axes for circular
-    orbits), using every host core.  Returns (projections/s, samples/s, cores, description,
-    ids, values, mfl, pathlen, margins)."""
+def oracle_sample(cfg, geom, vol_np, max_seconds=20.0, kernel=0, threads=None):
+    """Time the oracle, as it stands, on a bounded sample of the workload: whole detector rows of eight
+    projections spread over the orbit (both driving axes and the switches between them for circular
+    orbits), on `threads` host threads (default: every core).  Returns (projections/s, samples/s, cores,
+    description, ids, values, mfl, pathlen, margins)."""
     import oracle
-    cores = oracle.host_cores()
+    cores = oracle.host_cores() if threads is None else threads
     # eight poses spread over the orbit: both driving axes, both signs, and the switches between them
     projs = sorted({(k * cfg.n_proj) // 8 + (cfg.n_proj // 16 if k % 2 else 0) for k in range(8)})
     # calibrate on a few rows, then size the sample for ~max_seconds of wall time
@@ -234,12 +253,13 @@ def run_backproject(args, torch, fp, cfg, geom, vol, proj, P, stream, world, ran
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--config", default="C3", choices=["C1", "C2", "C3", "C4", "C5", "P1"])
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-probes", action="store_true", help="skip the L2 / shared-memory read probes")
     ap.add_argument("--kernel", type=int, default=0, help="FP_OPT_KERNEL value (0 = auto)")
     ap.add_argument("--group", type=int, default=-1, help="FP_OPT_GROUP (-1 = library default)")
     ap.add_argument("--op", default="project", choices=["project", "backproject"],
@@ -251,6 +271,15 @@ def main():
     if args.impl == "reference":
         return run_reference(args)
     args.warmup = max(args.warmup, 3)          # timing rule: at least three untimed warm-up steps
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        # python bench.py --gpus N: start the N replicas ourselves, one process per GPU
+        import socket
+        with socket.socket() as sk:
+            sk.bind(("127.0.0.1", 0))
+            port = sk.getsockname()[1]
+        cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", str(args.gpus),
+               "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+        return subprocess.call(cmd)
 
     import torch
     from paper_1609_00958_b200 import fp, synth
@@ -301,11 +330,12 @@ def main():
     # sample count of one step (outside the timed region: fp_last_sample_count synchronises, and the
     # count costs one exact fp64 ray set-up per ray that the sampling itself does not need)
     samples = 0
+    P.set_option(fp.OPT_COUNT_SAMPLES, 1)
     for p0 in range(0, cfg.n_proj, batch):
         p1 = min(cfg.n_proj, p0 + batch)
         P.project(vol, geom[p0:p1], cfg.nu, cfg.nv, out=out[p0:p1], stream=stream)
         samples += P.last_sample_count()
-    P.set_option(fp.OPT_COUNT_SAMPLES, 0)
+    P.set_option(fp.OPT_COUNT_SAMPLES, 0)        # the library default: the timed path is the one a user gets
     for _ in range(args.warmup):
         step()
     torch.cuda.synchronize()
@@ -323,6 +353,7 @@ def main():
     torch.cuda.synchronize()
     barrier()
     clk = clocks.stop()
+    P.check()                                    # no kernel found the host plan too small
     step_ms = [ev[k].elapsed_time(ev[k + 1]) for k in range(args.steps)]
     total_ms = ev[0].elapsed_time(ev[args.steps])
     total_ms = max_over_ranks(dist, total_ms)
@@ -371,13 +402,42 @@ def main():
     peaks, peak_kind = measured_peaks()
     vol_bytes = vol.numel() * 4
     out_bytes_per_proj = cfg.nu * cfg.nv * 4
-    # algorithmic HBM bytes per projection: the volume once + the projection written once
-    algo_bytes_per_step = cfg.n_proj * (vol_bytes + out_bytes_per_proj)
-    kernel_ms = ms_per_step            # one sampling launch per fp_project; the step is that launch
+    # algorithmic HBM bytes per projection: the voxels the cone can touch once + the projection written once
+    # (DESIGN.md).  With FP_OPT_FOV_CYLINDER the method's own work is the inscribed cylinder, pi/4 of the box.
+    vol_algo = vol_bytes * (math.pi / 4.0 if cfg.cylinder else 1.0)
+    algo_bytes_per_step = cfg.n_proj * (vol_algo + out_bytes_per_proj)
+    n_calls = max(1, (cfg.n_proj + batch - 1) // batch)
+    kernel_ms = ms_per_step            # one sampling launch per fp_project; the step is that launch (or n_calls of them)
     achieved = algo_bytes_per_step / (kernel_ms * 1e-3) / 1e9
+    cap, stale = captured_traffic(cfg.name, kernel_name, args.interp)
+    use = cap is not None and not stale
     roofline = {"bound": "hbm", "achieved": achieved, "peak": peaks["hbm_gbs"], "unit": "GB/s",
-                "frac": achieved / peaks["hbm_gbs"], "traffic": NCU_TRAFFIC_BYTES.get((cfg.name, kernel_name)), "peak_kind": peak_kind,
-                "kernel": kernel_name, "projections_per_kernel": kernel_share, "algorithmic_bytes_per_launch": algo_bytes_per_step // max(1, (cfg.n_proj + batch - 1) // batch)}
+                "frac": achieved / peaks["hbm_gbs"],
+                "traffic": cap["dram_bytes"] if use else None,
+                "traffic_source": (cap["source"] if use else ("stale: sources changed since " + cap["source"] if cap else None)),
+                "peak_kind": peak_kind, "kernel": kernel_name, "projections_per_kernel": kernel_share,
+                "algorithmic_bytes_per_launch": algo_bytes_per_step / n_calls,
+                "algorithmic_bytes_note": ("volume bytes x pi/4 (inscribed cylinder, FP_OPT_FOV_CYLINDER) + projection bytes"
+                                           if cfg.cylinder else "volume bytes + projection bytes, per projection"),
+                "median_ms": statistics.median(step_ms), "best_ms": min(step_ms),
+                "frac_best": algo_bytes_per_step / (min(step_ms) * 1e-3) / 1e9 / peaks["hbm_gbs"]}
+    # L2 and L1 / shared-memory rates against probed peaks (BASELINE.json metric: "achieved HBM/L2 GB/s vs peak")
+    roofline_l2 = roofline_l1 = None
+    if not args.no_probes:
+        l2_peak = fp.probe_bandwidth(fp.PROBE_L2_READ)
+        sh_peak = fp.probe_bandwidth(fp.PROBE_SHARED_READ)
+        hbm_read = fp.probe_bandwidth(fp.PROBE_HBM_READ)
+        l2_ach = (cap["l2_bytes"] / (kernel_ms / n_calls * 1e-3) / 1e9) if use and cap.get("l2_bytes") else None
+        roofline_l2 = {"bound": "l2", "achieved": l2_ach, "peak": l2_peak, "unit": "GB/s",
+                       "frac": (l2_ach / l2_peak) if l2_ach else None,
+                       "achieved_kind": "32 B x lts__t_sectors_srcunit_tex of the kept ncu capture / live kernel time" if l2_ach else "no current capture",
+                       "peak_kind": "fp_probe_bandwidth(L2_READ): 48 MiB re-read through ld.global.cg", "hbm_read_probe_gbs": hbm_read}
+        tap_gbs = TAP_BYTES * samples_per_s / world / 1e9
+        sh_ach = (cap["lsu_wavefronts"] * 128.0 / (kernel_ms / n_calls * 1e-3) / 1e9) if use and cap.get("lsu_wavefronts") else None
+        roofline_l1 = {"bound": "shared", "achieved": tap_gbs, "peak": sh_peak, "unit": "GB/s", "frac": tap_gbs / sh_peak,
+                       "achieved_kind": "16 B x samples / time: the four taps of every sample (PAPER.md:314)",
+                       "wavefront_gbs": sh_ach, "wavefront_frac": (sh_ach / sh_peak) if sh_ach else None,
+                       "peak_kind": "fp_probe_bandwidth(SHARED_READ): conflict-free 32-bit loads"}
 
     cpu_baseline = None
     parity = None
@@ -386,10 +446,22 @@ def main():
         pps, sps, cores, desc, ids, val, mfl, pl, mg = oracle_sample(cfg, geom, vol_np, max_seconds=15.0, kernel=1 if args.interp == "spline" else 0)
         cpu_baseline = {"value": pps, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc,
                         "gsamples_per_s": sps / 1e9, "extrapolated_from_sample": True}
+        # the same oracle on ONE thread, on a sample a tenth as long
+        pps1, sps1, _, desc1, *_ = oracle_sample(cfg, geom, vol_np, max_seconds=4.0, kernel=1 if args.interp == "spline" else 0, threads=1)
+        cpu_baseline["single_thread"] = {"value": pps1, "unit": UNIT, "cores": 1, "gsamples_per_s": sps1 / 1e9, "sample": desc1}
         g = out[torch.from_numpy(ids[:, 0].astype(np.int64)).cuda(), torch.from_numpy(ids[:, 1].astype(np.int64)).cuda(),
                 torch.from_numpy(ids[:, 2].astype(np.int64)).cuda()].cpu().numpy().astype(np.float64)
         tol = 2e-5 * np.abs(val) + 1e-6 * pl * float(vol.abs().max().item())
-        parity = {"rays": int(len(ids)), "worst_err_over_tol": float(np.max(np.abs(g - val) / np.maximum(tol, 1e-300)))}
+        gm = P.ray_ranges(geom, cfg.nu, cfg.nv) if cfg.n_proj * cfg.nu * cfg.nv <= (1 << 28) else None
+        idx_equal = None
+        if gm is not None:
+            gmr = gm[torch.from_numpy(ids[:, 0].astype(np.int64)).cuda(), torch.from_numpy(ids[:, 1].astype(np.int64)).cuda(),
+                     torch.from_numpy(ids[:, 2].astype(np.int64)).cuda()].cpu().numpy()
+            idx_equal = bool(np.array_equal(gmr, mfl))
+            del gm
+        miss = mfl[:, 2] < mfl[:, 1]
+        parity = {"rays": int(len(ids)), "worst_err_over_tol": float(np.max(np.abs(g - val) / np.maximum(tol, 1e-300))),
+                  "indices_equal": idx_equal, "misses_are_plus_zero": bool(np.all(g[miss] == 0.0) and not np.signbit(g[miss]).any())}
 
     line = {
         "metric": METRIC, "value": proj_per_s, "unit": UNIT, "n_gpus": world, "steps": args.steps,
@@ -403,10 +475,14 @@ def main():
         "samples_per_step": samples,
         "tap_access_rate_gbs": TAP_BYTES * samples_per_s / 1e9,
         "step_ms": step_ms,
+        "ms_median": statistics.median(step_ms), "ms_best": min(step_ms),
+        "value_best": replicas_throughput(world, cfg.n_proj, min(step_ms) * 1e-3),
         "clocks": clk,
         "gpu_launches": launches,
         "e2e": e2e,
         "roofline": roofline,
+        "roofline_l2": roofline_l2,
+        "roofline_l1": roofline_l1,
         "cpu_baseline": cpu_baseline,
         "parity_check": parity,
         "paper_context": "GTX 970: 176 projections/s (GJP_lin, global memory), 292 GB/s tap access rate, "

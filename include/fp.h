@@ -96,7 +96,8 @@ enum {
      * 0: z-driven rays read the caller's layout with strided taps. */
     FP_OPT_PERMUTED_COPY = 4,
     /* 1: fp_project accumulates the number of samples sum(i_last - i_first + 1) for
-     * fp_last_sample_count (default 1; one atomic per thread block). */
+     * fp_last_sample_count (default 0: the count costs one exact fp64 ray set-up per ray that the
+     * aligned / TMA sampling kernels do not otherwise need). */
     FP_OPT_COUNT_SAMPLES = 5,
     /* 1: the caller promises that the volume is ZERO outside the cylinder about the z axis through the grid
      * centre ((nx-1)/2, (ny-1)/2) with diameter min(nx, ny) voxels (the paper's benchmark object: "a cylindric
@@ -215,6 +216,19 @@ fp_status fp_plan(fp_ctx *ctx, const double *geom_host, int nu, int nv, int *ker
 
 /* fp_last_launch_count: how many kernels of this library the most recent fp_project enqueued. */
 fp_status fp_last_launch_count(fp_ctx *ctx, int *n);
+
+/*
+ * fp_probe_bandwidth: read-bandwidth probes of the measurement harness (the L2 and
+ * L1 / shared-memory peaks come from a read microbenchmark in the harness, no published figure is relied on;
+ * the paper's own metric is a cache-level access rate).  Runs a small kernel on the current
+ * device's default stream, synchronises, and returns the best of five runs in GB/s (1e9 bytes per second):
+ *   FP_PROBE_HBM_READ     a 2 GiB buffer streamed once through L2 only (ld.global.cg)
+ *   FP_PROBE_L2_READ      a 48 MiB buffer (resident in L2) streamed 64 times the same way
+ *   FP_PROBE_SHARED_READ  conflict-free 32-bit shared-memory loads, the access the sampling kernels make
+ * Needs no context.  FP_ERR_OOM if the buffer cannot be allocated.
+ */
+enum { FP_PROBE_HBM_READ = 0, FP_PROBE_L2_READ = 1, FP_PROBE_SHARED_READ = 2 };
+fp_status fp_probe_bandwidth(int what, double *gbs);
 
 const char *fp_status_string(fp_status s);
 const char *fp_last_error(fp_ctx *ctx);

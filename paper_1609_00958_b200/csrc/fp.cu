@@ -16,6 +16,7 @@
 #include "fp_aligned.cuh"
 #include "fp_tma.cuh"
 #include "fp_tex.cuh"
+#include "fp_probe.cuh"
 
 using namespace fpk;
 
@@ -26,7 +27,7 @@ struct fp_ctx {
     int opt_volatile = 1;
     int opt_interp = FP_INTERP_LINEAR;
     int opt_permuted = 1;
-    int opt_count = 1;
+    int opt_count = 0;
     int opt_fov = 0;
     int opt_group = 8;                         // projections per launch-order group of the aligned / TMA kernels
     int opt_force_tma = 0;                     // test hook: every aligned pose goes to fp_tma_kernel whether it fits or not
@@ -960,4 +961,55 @@ extern "C" fp_status fp_project_host(fp_ctx *c, const float *vol_host, int n_pro
     }
     if (h[1] != 0) return fail(c, FP_ERR_UNSUPPORTED, kPlanError);
     return FP_OK;
+}
+
+// Read-bandwidth probes of the measurement harness (fp_probe.cuh): best of five timed runs, CUDA events.
+extern "C" fp_status fp_probe_bandwidth(int what, double *gbs)
+{
+    if (!gbs) return FP_ERR_INVALID_ARG;
+    *gbs = 0.0;
+    if (what != FP_PROBE_HBM_READ && what != FP_PROBE_L2_READ && what != FP_PROBE_SHARED_READ) return FP_ERR_INVALID_ARG;
+    int dev = 0, n_sm = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) {
+        cudaGetLastError();
+        return FP_ERR_CUDA;
+    }
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
+    float *buf = nullptr, *sink = nullptr;
+    fp_status st = FP_OK;
+    double best = 0.0;
+    // HBM: 2 GiB streamed once per run; L2: 48 MiB (well inside the 126 MB L2) streamed 64 times per run
+    const size_t bytes = what == FP_PROBE_HBM_READ ? ((size_t)2 << 30) : ((size_t)48 << 20);
+    const int reps = what == FP_PROBE_HBM_READ ? 1 : 64, iters = 4096;
+    do {
+        if (cudaEventCreate(&e0) != cudaSuccess || cudaEventCreate(&e1) != cudaSuccess ||
+            cudaMalloc(&sink, sizeof(float)) != cudaSuccess) { st = FP_ERR_CUDA; break; }
+        if (what != FP_PROBE_SHARED_READ) {
+            if (cudaMalloc(&buf, bytes) != cudaSuccess) { st = FP_ERR_OOM; break; }
+            if (cudaMemset(buf, 0, bytes) != cudaSuccess) { st = FP_ERR_CUDA; break; }
+        }
+        for (int run = 0; run < 6 && st == FP_OK; ++run) {          // run 0 warms up
+            cudaEventRecord(e0, 0);
+            double moved = 0.0;
+            if (what == FP_PROBE_SHARED_READ) {
+                fp_probe_shared_kernel<<<n_sm * 2, 1024>>>(iters, sink);
+                moved = (double)n_sm * 2 * 1024 * (double)iters * 16 * 4;
+            } else {
+                fp_probe_read_kernel<<<n_sm * 4, 512>>>(reinterpret_cast<const float4 *>(buf), bytes / 16, reps, sink);
+                moved = (double)bytes * reps;
+            }
+            cudaEventRecord(e1, 0);
+            if (cudaEventSynchronize(e1) != cudaSuccess || cudaGetLastError() != cudaSuccess) { st = FP_ERR_CUDA; break; }
+            float ms = 0.f;
+            cudaEventElapsedTime(&ms, e0, e1);
+            if (run > 0 && ms > 0.f) best = std::max(best, moved / (ms * 1e-3) / 1e9);
+        }
+    } while (false);
+    cudaFree(buf);
+    cudaFree(sink);
+    if (e0) cudaEventDestroy(e0);
+    if (e1) cudaEventDestroy(e1);
+    cudaGetLastError();
+    *gbs = best;
+    return st;
 }

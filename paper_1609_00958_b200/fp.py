@@ -26,7 +26,8 @@ INTERP_LINEAR, INTERP_SPLINE = 0, 1
 # every symbol include/fp.h declares (tests check the library exports all of them)
 SYMBOLS = ["fp_create", "fp_destroy", "fp_set_option", "fp_get_option", "fp_prepare", "fp_project",
            "fp_project_host", "fp_backproject", "fp_ray_ranges", "fp_plan", "fp_check", "fp_last_sample_count",
-           "fp_last_launch_count", "fp_status_string", "fp_last_error", "fp_version"]
+           "fp_last_launch_count", "fp_probe_bandwidth", "fp_status_string", "fp_last_error", "fp_version"]
+PROBE_HBM_READ, PROBE_L2_READ, PROBE_SHARED_READ = 0, 1, 2
 
 
 class FpError(RuntimeError):
@@ -67,6 +68,8 @@ def load(build_if_missing: bool = True):
     L.fp_last_sample_count.argtypes = [vp, ctypes.POINTER(ctypes.c_ulonglong)]
     L.fp_last_launch_count.argtypes = [vp, ctypes.POINTER(i)]
     L.fp_check.argtypes = [vp]
+    L.fp_probe_bandwidth.argtypes = [i, ctypes.POINTER(ctypes.c_double)]
+    L.fp_probe_bandwidth.restype = i
     for name in ("fp_create", "fp_destroy", "fp_set_option", "fp_get_option", "fp_prepare", "fp_project", "fp_check",
                  "fp_project_host", "fp_backproject", "fp_ray_ranges", "fp_plan", "fp_last_sample_count", "fp_last_launch_count"):
         getattr(L, name).restype = i
@@ -233,6 +236,15 @@ class Projector:
         n = ctypes.c_int()
         self._check(self._L.fp_last_launch_count(self._h, ctypes.byref(n)))
         return n.value
+
+
+def probe_bandwidth(what: int) -> float:
+    """fp_probe_bandwidth: GB/s of the harness's read probe `what` (PROBE_*) on the current device."""
+    v = ctypes.c_double()
+    st = load().fp_probe_bandwidth(int(what), ctypes.byref(v))
+    if st != 0:
+        raise FpError(st, "fp_probe_bandwidth(%d)" % what)
+    return v.value
 
 
 def version() -> str:

@@ -40,6 +40,7 @@ def all_ids(n_proj, nv, nu, projs=None):
 def run_gpu(torch, fp, vol_np, delta, origin, geom, nu, nv, options=()):
     vol = torch.from_numpy(np.ascontiguousarray(vol_np, dtype=np.float32)).cuda()
     with fp.Projector(*vol_np.shape, delta, origin) as P:
+        P.set_option(fp.OPT_COUNT_SAMPLES, 1)
         for k, v in options:
             P.set_option(k, v)
         out = P.project(vol, geom, nu, nv)
@@ -114,6 +115,7 @@ def _big_config_subset(torch, fp, synth, oracle, name, projs, n_random, batch=No
     geom = synth.make_geometry(cfg)
     sub = geom[projs]
     with fp.Projector(*cfg.n, cfg.voxel_size, cfg.origin) as P:
+        P.set_option(fp.OPT_COUNT_SAMPLES, 1)
         for k, v in options:
             P.set_option(k, v)
         out = P.project(vol_t, sub, cfg.nu, cfg.nv)
@@ -288,6 +290,7 @@ def test_project_host_matches_device_path(torch, fp, synth):
     vol = synth.make_volume(cfg)
     geom = synth.make_geometry(cfg)
     with fp.Projector(*cfg.n, cfg.voxel_size, cfg.origin) as P:
+        P.set_option(fp.OPT_COUNT_SAMPLES, 1)
         a = P.project(vol.cuda(), geom, cfg.nu, cfg.nv).cpu()
         n1 = P.last_sample_count()
         b = P.project_host(vol.pin_memory(), geom, cfg.nu, cfg.nv)
@@ -431,14 +434,14 @@ def test_tma_kernel_c3_sampled_and_fallback(torch, fp, synth, oracle):
         assert all(P.plan(g, cfg.nu, cfg.nv)[0] == fp.KERNEL_TMA for g in geom)
         out = P.project(vol_t, geom, cfg.nu, cfg.nv)
         torch.cuda.synchronize()
-        P.last_sample_count()                  # raises if a window or row tile overflowed
+        P.check()                              # raises if a window or row tile overflowed
         out = out.cpu().numpy()
         # a pose that does not fit the tile (coarse detector columns) silently uses the aligned kernel
         coarse = aligned_pose(0.8, cfg.sid, cfg.sdd, 96, 64, 3.0)
         assert P.plan(coarse, 96, 64)[0] == fp.KERNEL_ALIGNED
         P.project(vol_t, coarse[None], 96, 64)
         torch.cuda.synchronize()
-        P.last_sample_count()
+        P.check()
     vol = vol_t.cpu().numpy()
     rng = np.random.default_rng(99)
     n = 30000
