@@ -260,6 +260,8 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-probes", action="store_true", help="skip the L2 / shared-memory read probes")
+    ap.add_argument("--layout-prepared", action="store_true",
+                    help="FP_OPT_VOLATILE = 0 and fp_prepare before the timed region: the layout stage is NOT timed")
     ap.add_argument("--kernel", type=int, default=0, help="FP_OPT_KERNEL value (0 = auto)")
     ap.add_argument("--group", type=int, default=-1, help="FP_OPT_GROUP (-1 = library default)")
     ap.add_argument("--op", default="project", choices=["project", "backproject"],
@@ -311,6 +313,9 @@ def main():
     if cfg.cylinder:
         P.set_option(fp.OPT_FOV_CYLINDER, 1)       # the volume is zero outside the inscribed cylinder
     stream = torch.cuda.current_stream()
+    if args.layout_prepared:
+        P.set_option(fp.OPT_VOLATILE, 0)
+        P.prepare(vol, stream=stream)
 
     if args.op == "backproject":
         return run_backproject(args, torch, fp, cfg, geom, vol, out, P, stream, world, rank, dist)
@@ -395,7 +400,8 @@ def main():
 
     # which sampling kernel the library's plan picks for this workload (fp_plan, host only)
     plans = [P.plan(g, cfg.nu, cfg.nv)[0] for g in geom]
-    names = {fp.KERNEL_DIRECT: "fp_direct_kernel", fp.KERNEL_ALIGNED: "fp_aligned_kernel", fp.KERNEL_TMA: "fp_tma_kernel"}
+    names = {fp.KERNEL_DIRECT: "fp_direct_kernel", fp.KERNEL_ALIGNED: "fp_aligned_kernel", fp.KERNEL_TMA: "fp_tma_kernel",
+             fp.KERNEL_TEX: "fp_tex_kernel", fp.KERNEL_HWLIN: "fp_tex_kernel (hardware filtering)"}
     # every pose is planned on its own; name the kernel that takes most of them and say how many
     kernel_name = names[max(set(plans), key=plans.count)]
     kernel_share = {names[k]: plans.count(k) for k in sorted(set(plans))}
@@ -470,7 +476,7 @@ def main():
         "config": {"workload": workload_name(cfg), "projections_per_call": batch, "replicas": world,
                    "l2_policy": "inputs larger than L2 (volume %d MB, output %d MB per step; L2 126 MB)" % (
                        vol_bytes >> 20, (cfg.n_proj * out_bytes_per_proj) >> 20),
-                   "layout_stage_in_timed_region": True, "interpolation": args.interp},
+                   "layout_stage_in_timed_region": not args.layout_prepared, "interpolation": args.interp},
         "gsamples_per_s": samples_per_s / 1e9,
         "samples_per_step": samples,
         "tap_access_rate_gbs": TAP_BYTES * samples_per_s / 1e9,

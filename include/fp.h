@@ -205,8 +205,8 @@ fp_status fp_check(fp_ctx *ctx);
 
 /*
  * fp_plan: the host-side plan fp_project makes for ONE pose (no device needed, nothing is launched):
- *   *kernel    FP_KERNEL_ALIGNED, FP_KERNEL_TMA or FP_KERNEL_DIRECT: the sampling kernel this pose gets
- *              under the current FP_OPT_KERNEL
+ *   *kernel    FP_KERNEL_ALIGNED, FP_KERNEL_TMA, FP_KERNEL_DIRECT (or FP_KERNEL_TEX / FP_KERNEL_HWLIN when one
+ *              of those is forced): the sampling kernel this pose gets under the current FP_OPT_KERNEL
  *   *window    staging window of the aligned kernel in voxels along z (0 for the direct kernel)
  *   *z_driven  1 if some ray of the pose has z as its driving axis (Eq. 2), which is
  *              what makes fp_project build the permuted copy of the layout stage

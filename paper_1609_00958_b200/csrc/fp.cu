@@ -866,6 +866,10 @@ extern "C" fp_status fp_plan(fp_ctx *c, const double *geom, int nu, int nv, int 
     *kernel = al ? FP_KERNEL_ALIGNED : FP_KERNEL_DIRECT;
     if (al && c->opt_kernel != FP_KERNEL_ALIGNED && fits_tma(w, rows)) *kernel = FP_KERNEL_TMA;
     *window = al ? w : 0;
+    if (c->opt_kernel == FP_KERNEL_TEX || c->opt_kernel == FP_KERNEL_HWLIN) {
+        *kernel = c->opt_kernel;                           // every pose goes through the texture pipe
+        *window = 0;
+    }
     *z_driven = has_z_driven(geom, nu, nv) ? 1 : 0;
     return FP_OK;
 }
