@@ -401,7 +401,7 @@ def main():
     # which sampling kernel the library's plan picks for this workload (fp_plan, host only)
     plans = [P.plan(g, cfg.nu, cfg.nv)[0] for g in geom]
     names = {fp.KERNEL_DIRECT: "fp_direct_kernel", fp.KERNEL_ALIGNED: "fp_aligned_kernel", fp.KERNEL_TMA: "fp_tma_kernel",
-             fp.KERNEL_TEX: "fp_tex_kernel", fp.KERNEL_HWLIN: "fp_tex_kernel (hardware filtering)"}
+             fp.KERNEL_TEX: "fp_tex_kernel", fp.KERNEL_TILE: "fp_tile_kernel", fp.KERNEL_HWLIN: "fp_tex_kernel (hardware filtering)"}
     # every pose is planned on its own; name the kernel that takes most of them and say how many
     kernel_name = names[max(set(plans), key=plans.count)]
     kernel_share = {names[k]: plans.count(k) for k in sorted(set(plans))}

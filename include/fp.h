@@ -67,8 +67,10 @@ typedef enum {
 enum {
     /* Sampling-kernel variant.  Poses whose v vector is parallel to the volume's z axis, whose u vector is
      * perpendicular to it and that have no z-driven ray (every circular orbit about z)
-     * are "aligned"; all other poses always use FP_KERNEL_DIRECT (one thread per ray, four global taps per
-     * sample).  For each aligned pose (one launch per kernel and call):
+     * are "aligned"; all other poses use FP_KERNEL_TILE (32 x 16 pixel tiles whose slice footprints the TMA engine
+     * copies to shared memory; needs nz % 4 == 0 and a 16-byte aligned volume) or, failing that or when forced,
+     * FP_KERNEL_DIRECT (one thread per ray, four global taps per sample).  For each aligned pose (one launch per
+     * kernel and call):
      *   FP_KERNEL_AUTO     FP_KERNEL_TMA if the pose fits a 256-voxel z window and 12 volume rows per block
      *                      and slice, else FP_KERNEL_ALIGNED;
      *   FP_KERNEL_TMA      the same as AUTO (tiles of the caller's volume copied to shared memory by
@@ -76,6 +78,7 @@ enum {
      *   FP_KERNEL_ALIGNED  always the line-staging kernel (two volume rows blended into shared memory per
      *                      column and slice, two taps per sample);
      *   FP_KERNEL_DIRECT   the direct kernel for every pose;
+     *   FP_KERNEL_TILE     the same as AUTO;
      *   FP_KERNEL_TEX      every pose (aligned or not) through the texture pipe: the layout stage copies the
      *                      volume into one layered 2-D array per driving axis in use (brick-tiled texel order,
      *                      PAPER.md:290-294), one tld4 per sample returns the four taps, explicit fp32 weights;
@@ -116,7 +119,8 @@ enum {
     FP_OPT_TEST_FORCE_TMA = 100
 };
 
-enum { FP_KERNEL_AUTO = 0, FP_KERNEL_DIRECT = 1, FP_KERNEL_ALIGNED = 2, FP_KERNEL_TMA = 3, FP_KERNEL_TEX = 4, FP_KERNEL_HWLIN = 5 };
+enum { FP_KERNEL_AUTO = 0, FP_KERNEL_DIRECT = 1, FP_KERNEL_ALIGNED = 2, FP_KERNEL_TMA = 3, FP_KERNEL_TEX = 4, FP_KERNEL_HWLIN = 5,
+       FP_KERNEL_TILE = 6 };
 enum { FP_INTERP_LINEAR = 0, FP_INTERP_SPLINE = 1 };
 
 /*
@@ -205,7 +209,7 @@ fp_status fp_check(fp_ctx *ctx);
 
 /*
  * fp_plan: the host-side plan fp_project makes for ONE pose (no device needed, nothing is launched):
- *   *kernel    FP_KERNEL_ALIGNED, FP_KERNEL_TMA, FP_KERNEL_DIRECT (or FP_KERNEL_TEX / FP_KERNEL_HWLIN when one
+ *   *kernel    FP_KERNEL_ALIGNED, FP_KERNEL_TMA, FP_KERNEL_TILE, FP_KERNEL_DIRECT (or FP_KERNEL_TEX / FP_KERNEL_HWLIN when one
  *              of those is forced): the sampling kernel this pose gets under the current FP_OPT_KERNEL
  *   *window    staging window of the aligned kernel in voxels along z (0 for the direct kernel)
  *   *z_driven  1 if some ray of the pose has z as its driving axis (Eq. 2), which is

@@ -16,6 +16,7 @@
 #include "fp_aligned.cuh"
 #include "fp_tma.cuh"
 #include "fp_tex.cuh"
+#include "fp_tile.cuh"
 #include "fp_probe.cuh"
 
 using namespace fpk;
@@ -45,6 +46,9 @@ struct fp_ctx {
     // tensor maps of the TMA kernel: valid for one volume pointer
     CUtensorMap tmap[2][kTmWBoxes][kTmMaps];
     const float *tmap_vol = nullptr;
+    // tensor maps of the tile kernel: [driving axis][box size]; axis 2 covers the y-fastest copy
+    CUtensorMap tlmap[3][kTlSizes];
+    const float *tlmap_vol = nullptr, *tlmap_perm = nullptr;
     // layout stage of fp_tex_kernel: one layered 2-D array per driving axis (layer = slice), its surface (fill
     // kernel) and two texture objects over it (point sampling for tld4, linear filtering for GJP_hwlin)
     cudaArray_t arr[3] = {nullptr, nullptr, nullptr};
@@ -199,7 +203,7 @@ extern "C" fp_status fp_set_option(fp_ctx *c, int key, int value)
     if (!c) return FP_ERR_INVALID_ARG;
     switch (key) {
     case FP_OPT_KERNEL:
-        if (value < FP_KERNEL_AUTO || value > FP_KERNEL_HWLIN) return fail(c, FP_ERR_INVALID_ARG, "bad kernel variant");
+        if (value < FP_KERNEL_AUTO || value > FP_KERNEL_TILE) return fail(c, FP_ERR_INVALID_ARG, "bad kernel variant");
         c->opt_kernel = value;
         return FP_OK;
     case FP_OPT_VOLATILE: c->opt_volatile = value != 0; return FP_OK;
@@ -424,17 +428,57 @@ typedef CUresult (*tensor_map_encode_fn)(CUtensorMap *, CUtensorMapDataType, cuu
                                          const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
                                          CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
 
-static fp_status build_tensor_maps(fp_ctx *c, const float *vol)
+static tensor_map_encode_fn g_encode = nullptr;
+
+static fp_status get_encoder(fp_ctx *c)
 {
-    if (c->tmap_vol == vol) return FP_OK;
-    static tensor_map_encode_fn encode = nullptr;
-    if (!encode) {
+    if (!g_encode) {
         void *fn = nullptr;
         cudaDriverEntryPointQueryResult q;
         FP_CUDA(c, cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &q));
         if (!fn || q != cudaDriverEntryPointSuccess) return fail(c, FP_ERR_UNSUPPORTED, "cuTensorMapEncodeTiled not available");
-        encode = (tensor_map_encode_fn)fn;
+        g_encode = (tensor_map_encode_fn)fn;
     }
+    return FP_OK;
+}
+
+// Tensor maps of fp_tile_kernel: per driving axis a rows x cols box of one slice plane, fast in-plane axis innermost.
+// m = x, y: the caller's volume, dimensions (z, y, x); m = z: the y-fastest copy [nz][nx][ny], dimensions (y, x, z).
+static fp_status build_tile_maps(fp_ctx *c, const float *vol, const float *perm)
+{
+    if (c->tlmap_vol == vol && c->tlmap_perm == perm) return FP_OK;
+    fp_status s = get_encoder(c);
+    if (s != FP_OK) return s;
+    const cuuint32_t estr[3] = {1, 1, 1};
+    for (int m = 0; m < 3; ++m) {
+        if (m == 2 && !perm) continue;
+        const cuuint64_t nx = c->G.n[0], ny = c->G.n[1], nz = c->G.n[2];
+        const cuuint64_t dims[3] = {m == 2 ? ny : nz, m == 2 ? nx : ny, m == 2 ? nz : nx};
+        const cuuint64_t strides[2] = {dims[0] * 4, dims[0] * dims[1] * 4};
+        for (int k = 0; k < kTlSizes; ++k) {
+            const cuuint32_t rows = (cuuint32_t)tl_rows(k), cols = (cuuint32_t)tl_cols(k);
+            const cuuint32_t box[3] = {cols, m == 1 ? 1u : rows, m == 1 ? rows : 1u};
+            const CUresult r = g_encode(&c->tlmap[m][k], CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, (void *)(m == 2 ? perm : vol), dims,
+                                        strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                                        CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+            if (r != CUDA_SUCCESS) {
+                char buf[96];
+                snprintf(buf, sizeof buf, "cuTensorMapEncodeTiled (tile kernel) failed (%d)", (int)r);
+                return fail(c, FP_ERR_CUDA, buf);
+            }
+        }
+    }
+    c->tlmap_vol = vol;
+    c->tlmap_perm = perm;
+    return FP_OK;
+}
+
+static fp_status build_tensor_maps(fp_ctx *c, const float *vol)
+{
+    if (c->tmap_vol == vol) return FP_OK;
+    fp_status es = get_encoder(c);
+    if (es != FP_OK) return es;
+    tensor_map_encode_fn encode = g_encode;
     const cuuint64_t dims[3] = {(cuuint64_t)c->G.n[2], (cuuint64_t)c->G.n[1], (cuuint64_t)c->G.n[0]};
     const cuuint64_t strides[2] = {(cuuint64_t)c->G.n[2] * 4, (cuuint64_t)c->G.n[2] * c->G.n[1] * 4};
     const cuuint32_t estr[3] = {1, 1, 1};
@@ -756,7 +800,37 @@ extern "C" fp_status fp_project(fp_ctx *c, const float *vol_dev, int n_proj, con
         c->last_launches += 1;
     }
 
-    if (!ids_di.empty()) {
+    // general poses: the TMA-staged tile kernel when the volume can be addressed by tensor maps (16-byte aligned
+    // base, row lengths that are multiples of 4 voxels), else -- or with FP_KERNEL_DIRECT -- the direct kernel
+    const bool tile_ok = c->opt_kernel != FP_KERNEL_DIRECT && ((uintptr_t)vol_dev & 15) == 0 && (c->G.n[2] & 3) == 0 &&
+                         (!use_perm || (c->G.n[1] & 3) == 0);
+    if (!ids_di.empty() && tile_ok) {
+        s = build_tile_maps(c, vol_dev, use_perm ? c->vol_perm : nullptr);
+        if (s != FP_OK) return s;
+        TileParams T;
+        memcpy(T.map, c->tlmap, sizeof T.map);
+        T.G = c->G;
+        fill_layouts(c, vol_dev, use_perm, T.lay);
+        T.proj = c->proj_dev;
+        T.ids = c->ids_dev + c->ids_cap;
+        T.out = out_dev;
+        T.sample_count = c->opt_count ? c->count_dev : nullptr;
+        T.nu = nu;
+        T.nv = nv;
+        T.n_sel = (int)ids_di.size();
+        T.z_staged = use_perm ? 1 : 0;
+        dim3 grid((unsigned)((nu + kTlU - 1) / kTlU), (unsigned)((nv + kTlV - 1) / kTlV), (unsigned)ids_di.size());
+        const size_t smem = tile_smem_bytes();
+        if (c->opt_interp == FP_INTERP_SPLINE) {
+            FP_CUDA(c, cudaFuncSetAttribute(fp_tile_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+            fp_tile_kernel<1><<<grid, kTlThreads, smem, st>>>(T);
+        } else {
+            FP_CUDA(c, cudaFuncSetAttribute(fp_tile_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+            fp_tile_kernel<0><<<grid, kTlThreads, smem, st>>>(T);
+        }
+        FP_CUDA(c, cudaGetLastError());
+        c->last_launches += 1;
+    } else if (!ids_di.empty()) {
         ProjectParams P;
         P.G = c->G;
         fill_layouts(c, vol_dev, use_perm, P.lay);
@@ -863,7 +937,7 @@ extern "C" fp_status fp_plan(fp_ctx *c, const double *geom, int nu, int nv, int 
     int rows = 0;
     const int w = c->opt_kernel == FP_KERNEL_DIRECT ? 0 : plan_aligned(c, nullptr, geom, nu, nv, &rows);
     const bool al = w > 0 && w <= kAlignedMaxW;
-    *kernel = al ? FP_KERNEL_ALIGNED : FP_KERNEL_DIRECT;
+    *kernel = al ? FP_KERNEL_ALIGNED : ((c->opt_kernel != FP_KERNEL_DIRECT && (c->G.n[2] & 3) == 0) ? FP_KERNEL_TILE : FP_KERNEL_DIRECT);
     if (al && c->opt_kernel != FP_KERNEL_ALIGNED && fits_tma(w, rows)) *kernel = FP_KERNEL_TMA;
     *window = al ? w : 0;
     if (c->opt_kernel == FP_KERNEL_TEX || c->opt_kernel == FP_KERNEL_HWLIN) {

@@ -1,0 +1,317 @@
+// fp_tile.cuh -- TMA-staged sampling kernel for GENERAL poses (any source / detector orientation, all three
+// driving axes): the same Alg. 1 as fp_direct_kernel, but the four taps of Eq. 15 (:165) come
+// from shared memory instead of four uncoalesced global loads per sample.
+//
+// A block owns a 32 x 16 tile of detector pixels (512 rays, two per consumer thread as one packed fp32x2
+// value).  If its four corner rays share the driving axis m (Eq. 2, :81) -- then every ray of the tile does,
+// the set { r : m(r) = m } being a convex cone -- the rays cut slice i of axis m inside the quadrilateral spanned by
+// the corner rays' intersection points (the map pixel -> intersection point is projective).  A producer warp
+// evaluates those four points per slice in fp64 (Eq. 6, :104) and has the TMA engine copy the bounding box of the
+// quadrilateral (rows x cols voxels of the slice plane, zero-filled outside the volume = reading #2; the fast
+// in-plane axis is the contiguous one: the caller's array for m = x, y, the y-fastest copy of the layout stage,
+// PAPER.md:290-294, for m = z) into a ring of shared-memory stages behind full / empty mbarriers.  The consumers
+// step through the block's slices together: position by one packed FMA per in-plane axis from an fp64 anchor
+// that is renewed every 64 slices (integer + fraction split, so the fp32 operands stay below 33 whatever the
+// volume size), floor by a round-down add, four shared-memory taps, product weights of Eq. 11 (:142).  A ray
+// outside its own slice range [i_first, i_last] has a transverse coordinate outside (-1, N_t), so all its taps
+// lie in the zero fill: no masks, no per-ray loop bounds.
+//
+// Tiles whose corner rays have different driving axes (about 4 % of C4's tiles), whose box would not fit the
+// largest stage, or whose rays all miss run the direct path (fp_kernels.cuh) inside the same launch.
+#pragma once
+#include <cstdint>
+#include <cuda.h>
+#include <cuda_runtime.h>
+#include "fp_setup.cuh"
+#include "fp_kernels.cuh"
+#include "fp_tma.cuh"
+
+namespace fpk {
+
+constexpr int kTlU = 32, kTlV = 16;              // detector pixels per block along u and v
+constexpr int kTlConsumers = kTlU * kTlV / 2;    // two rays per consumer thread
+constexpr int kTlThreads = kTlConsumers + 32;    // + one producer warp
+constexpr int kTlSizes = 3;                      // box sizes (rows x cols); cols % 32 = 4 or 20 words: rows fall in different banks
+__host__ __device__ constexpr int tl_rows(int k) { return k == 0 ? 28 : (k == 1 ? 44 : 60); }
+__host__ __device__ constexpr int tl_cols(int k) { return k == 0 ? 36 : (k == 1 ? 52 : 68); }
+constexpr int kTlStagesMax = 4;                  // four stages of the two smaller boxes, three of the largest
+// stage strides are multiples of 128 B (TMA destination alignment): 9216 >= 44 x 52 x 4, 16384 >= 60 x 68 x 4
+__host__ __device__ constexpr unsigned tl_stage_stride(int k) { return k == 2 ? 16384u : 9216u; }
+constexpr unsigned kTlTileBytes = 3u * 16384u;   // = 49152 >= 4 x 9216
+
+struct __align__(64) TileParams {
+    CUtensorMap map[3][kTlSizes];      // [driving axis][box size]
+    GridDesc G;
+    AxisLayout lay[3];                 // for the direct path of tiles that do not qualify
+    const ProjDesc *proj;              // all projections of the call
+    const int *ids;                    // [n_sel] projections this launch handles
+    float *out;                        // [n_proj][nv][nu]
+    unsigned long long *sample_count;  // may be null
+    int nu, nv, n_sel;
+    int z_staged;                      // 1: map[2] covers the y-fastest copy of the layout stage; 0: z-driven tiles run the direct path
+};
+
+struct TlCorner {                      // one corner ray, parametrised along the tile's driving axis
+    double s_m, s_a, s_b, rt_a, rt_b;
+};
+
+struct __align__(16) TlShared {
+    unsigned long long full[kTlStagesMax], empty[kTlStagesMax];
+    unsigned org[kTlStagesMax];        // per stage: byte address of tile word (0, 0) minus (js0 * pitch + kf0) * 4 terms, see below
+    TlCorner corner[4];
+    int m[4];                          // driving axis (+ 4 if r_m < 0) of the corner rays; -1: degenerate
+    int lo, hi;                        // slice range of the block (union of its rays' ranges)
+    int size, staged;                  // box size index; 1: staged path, 0: direct path
+};
+
+// Direct path for one ray (the body of fp_direct_kernel).
+template <int INTERP>
+__device__ __forceinline__ float tl_direct_ray(const RaySetup &R, const AxisLayout *lay)
+{
+    float acc = 0.0f;
+    if (R.i_last >= R.i_first) {
+        const AxisLayout &A = lay[R.m];
+        int in_lo = R.i_first, in_hi = R.i_last;
+        interior_clip(R.s_a, R.s_m, R.rt_a, 0.5, (double)A.n_s - 1.5, in_lo, in_hi);
+        if (in_lo <= in_hi) interior_clip(R.s_b, R.s_m, R.rt_b, 0.5, (double)A.n_f - 1.5, in_lo, in_hi);
+        if (in_lo <= in_hi) {
+            acc = direct_run<INTERP, true>(R, A, R.i_first, in_lo - 1);
+            acc += direct_run<INTERP, false>(R, A, in_lo, in_hi);
+            acc += direct_run<INTERP, true>(R, A, in_hi + 1, R.i_last);
+        } else {
+            acc = direct_run<INTERP, true>(R, A, R.i_first, R.i_last);
+        }
+    }
+    return acc;
+}
+
+template <int INTERP>
+__global__ void __launch_bounds__(kTlThreads, 2)
+fp_tile_kernel(const __grid_constant__ TileParams P)
+{
+    extern __shared__ __align__(128) unsigned char tl_smem_raw[];
+    TlShared &S = *reinterpret_cast<TlShared *>(tl_smem_raw + kTlTileBytes);
+    const unsigned tiles_smem = tm_smem(tl_smem_raw);
+
+    const int tid = threadIdx.x, lane = tid & 31;
+    const int warp = __shfl_sync(0xffffffffu, tid >> 5, 0);
+    const bool producer = warp == kTlConsumers / 32;
+    const int proj = P.ids[blockIdx.z];
+    const ProjDesc *pd = P.proj + proj;
+    const double *g = pd->g;
+    const int tu0 = blockIdx.x * kTlU, tv0 = blockIdx.y * kTlV;
+
+    // ---- corner rays (Eqs. 1-5): the tile's rectangle, also where it sticks out past the detector edge
+    if (tid < 4) {
+        const int iu = tu0 + ((tid & 1) ? kTlU - 1 : 0), iv = tv0 + ((tid & 2) ? kTlV - 1 : 0);
+        const RaySetup R = ray_setup(g, P.G, iu, iv);
+        TlCorner C;
+        C.s_m = R.s_m; C.s_a = R.s_a; C.s_b = R.s_b; C.rt_a = R.rt_a; C.rt_b = R.rt_b;
+        S.corner[tid] = C;
+        // driving axis AND sense of the corner ray: code m for r_m > 0, m + 4 for r_m < 0 (the rays between four
+        // corners lie in one convex cone { r : r_m >= |r_a| } only if the sense agrees as well)
+        const double rm = ((g[3 + R.m] + (double)iu * g[6 + R.m]) + (double)iv * g[9 + R.m]) - g[R.m];
+        S.m[tid] = R.L > 0.0 ? R.m + (rm < 0.0 ? 4 : 0) : -1;
+    }
+    if (tid == 0) {
+        S.lo = 0x7fffffff;
+        S.hi = -1;
+#pragma unroll
+        for (int k = 0; k < kTlStagesMax; ++k) {
+            tm_mbar_init(&S.full[k], 1);
+            tm_mbar_init(&S.empty[k], kTlConsumers / 32);
+        }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+
+    // ---- per-ray exact set-up (fp64, Eqs. 1-6 and the exact slice range); lanes run along the detector axis that
+    //      maps onto the contiguous in-plane axis of the tile's driving axis (neighbouring lanes -> neighbouring words)
+    const int m_code = S.m[0], m_tile = m_code & 3;
+    const bool same_m = m_code >= 0 && S.m[1] == m_code && S.m[2] == m_code && S.m[3] == m_code && (m_tile != 2 || P.z_staged);
+    const int fa = m_tile == 2 ? 1 : 2;                       // fast in-plane axis: z, or y on the permuted copy
+    const bool lanes_v = same_m && fabs(g[9 + fa]) > fabs(g[6 + fa]);
+    int iuA = 0, ivA = 0, iuB = 0, ivB = 0;
+    RaySetup RA, RB;
+    bool liveA = false, liveB = false;
+    if (!producer) {
+        const int w = tid >> 5;
+        if (!lanes_v) {                                       // 32 lanes along u; rows w and w + 8
+            iuA = iuB = tu0 + lane;
+            ivA = tv0 + w;
+            ivB = tv0 + w + 8;
+        } else {                                              // 16 lanes along v; two neighbouring columns per thread
+            ivA = ivB = tv0 + (lane & 15);
+            iuA = tu0 + 2 * (2 * w + (lane >> 4));
+            iuB = iuA + 1;
+        }
+        liveA = iuA < P.nu && ivA < P.nv;
+        liveB = iuB < P.nu && ivB < P.nv;
+        RA = ray_setup(g, P.G, min(iuA, P.nu - 1), min(ivA, P.nv - 1));
+        RB = ray_setup(g, P.G, min(iuB, P.nu - 1), min(ivB, P.nv - 1));
+        if (same_m) {
+            int lo = 0x7fffffff, hi = -1;
+            if (RA.i_last >= RA.i_first) { lo = RA.i_first; hi = RA.i_last; }
+            if (RB.i_last >= RB.i_first) { lo = min(lo, RB.i_first); hi = max(hi, RB.i_last); }
+            lo = __reduce_min_sync(0xffffffffu, lo);
+            hi = __reduce_max_sync(0xffffffffu, hi);
+            if (lane == 0 && hi >= lo) {
+                atomicMin(&S.lo, lo);
+                atomicMax(&S.hi, hi);
+            }
+        }
+    }
+    __syncthreads();
+    // ---- does the tile qualify for the staged path?  Box of the corner quadrilateral at both ends of the slice range
+    //      (every corner point is affine in the slice index, so the extents are largest at one of the ends)
+    if (tid == 0) {
+        int size = -1;
+        if (same_m && S.hi >= S.lo) {
+            int rows = 0, cols = 0;
+            for (int e = 0; e < 2; ++e) {
+                const int i = e ? S.hi : S.lo;
+                double smin = 1e300, smax = -1e300, fmin_ = 1e300, fmax_ = -1e300;
+                for (int c = 0; c < 4; ++c) {
+                    const TlCorner &C = S.corner[c];
+                    const double ps = p_of_i(C.s_a, C.s_m, C.rt_a, i), pf = p_of_i(C.s_b, C.s_m, C.rt_b, i);
+                    smin = fmin(smin, ps); smax = fmax(smax, ps);
+                    fmin_ = fmin(fmin_, pf); fmax_ = fmax(fmax_, pf);
+                }
+                // extent e of the positions: floor(max) - floor(min) <= floor(e) + 1 on any slice in between; rows
+                // floor(min) - 1 .. floor(max) + 2 are copied (one spare on either side of the taps)
+                rows = max(rows, (int)fmin(smax - smin, 1.0e6) + 5);
+                cols = max(cols, (int)fmin(fmax_ - fmin_, 1.0e6) + 8);     // + 3: the box starts on a 16-byte boundary
+            }
+            for (int k = kTlSizes - 1; k >= 0; --k)
+                if (rows <= tl_rows(k) && cols <= tl_cols(k)) size = k;
+        }
+        S.size = max(size, 0);
+        S.staged = size >= 0;
+    }
+    __syncthreads();
+
+    int n_samples = 0;
+    if (!S.staged) {
+        // ---- direct path (mixed driving axes, oversized box, or nothing to sample)
+        if (!producer) {
+            const float a = tl_direct_ray<INTERP>(RA, P.lay), b = tl_direct_ray<INTERP>(RB, P.lay);
+            if (liveA) P.out[((size_t)proj * P.nv + ivA) * P.nu + iuA] = (float)(P.G.delta * RA.L) * a;
+            if (liveB) P.out[((size_t)proj * P.nv + ivB) * P.nu + iuB] = (float)(P.G.delta * RB.L) * b;
+            if (liveA) n_samples += max(RA.i_last - RA.i_first + 1, 0);
+            if (liveB) n_samples += max(RB.i_last - RB.i_first + 1, 0);
+        }
+    } else {
+        const int lo = S.lo, hi = S.hi, size = S.size;
+        const int n_slices = hi - lo + 1;
+        const int nst = size == 2 ? 3 : 4;                               // stages in flight
+        const int rows = tl_rows(size), cols = tl_cols(size);
+        const unsigned pitchB = (unsigned)cols * 4u, boxB = (unsigned)(rows * cols * 4), stageB = tl_stage_stride(size);
+        if (producer) {
+            // lane = slice-in-batch * 8 + corner * 2 + coordinate; batches of four slices
+            const int sb = lane >> 3, cc = (lane >> 1) & 3, co = lane & 1;
+            const TlCorner C = S.corner[cc];
+            const double s_t = co ? C.s_b : C.s_a, rt_t = co ? C.rt_b : C.rt_a;
+            const CUtensorMap *map = &P.map[m_tile][size];
+            int st = 0;
+            unsigned ph = 0;                                             // parity of the empty phase to wait for (from the second round on)
+            for (int n0 = 0; n0 < n_slices; n0 += 4) {
+                const int i = lo + n0 + sb;
+                const double p = p_of_i(s_t, C.s_m, rt_t, min(i, hi));
+                double pmin = p;
+                pmin = fmin(pmin, __shfl_xor_sync(0xffffffffu, pmin, 2));
+                pmin = fmin(pmin, __shfl_xor_sync(0xffffffffu, pmin, 4));
+                // first row / column of the box: one spare on the low side for fp32 rounding of the consumers' positions;
+                // the first column on a 16-byte boundary of the volume's rows (the TMA engine traps otherwise)
+                const int o_t = co ? ((__double2int_rd(pmin) - 1) & ~3) : (__double2int_rd(pmin) - 1);
+                const int js0_l = __shfl_sync(0xffffffffu, o_t, 8 * sb), kf0_l = __shfl_sync(0xffffffffu, o_t, 8 * sb + 1);
+                for (int q = 0; q < 4 && n0 + q < n_slices; ++q) {
+                    const int n = n0 + q;
+                    const int js0 = __shfl_sync(0xffffffffu, js0_l, 8 * q), kf0 = __shfl_sync(0xffffffffu, kf0_l, 8 * q);
+                    if (n >= nst) tm_mbar_wait(&S.empty[st], ph);
+                    if (lane == 0) {
+                        // consumers add bits(row) * pitch + bits(col) * 4 with bits = 0x4B400000 + index (mod 2^32)
+                        S.org[st] = tiles_smem + st * stageB - ((0x4B400000u + (unsigned)js0) * pitchB + ((0x4B400000u + (unsigned)kf0) << 2));
+                        tm_mbar_arrive_tx(&S.full[st], boxB);
+                        const unsigned dst = tiles_smem + st * stageB;
+                        const int ii = lo + n;
+                        // tensor dimensions, fastest first: m = x: (z, y, x); m = y: (z, y, x) with the slow axis x;
+                        // m = z: the y-fastest copy (y, x, z)
+                        if (m_tile == 1)
+                            tm_load_3d(map, dst, &S.full[st], kf0, ii, js0);
+                        else
+                            tm_load_3d(map, dst, &S.full[st], kf0, js0, ii);
+                    }
+                    __syncwarp();
+                    if (++st == nst) {
+                        st = 0;
+                        if (n >= nst) ph ^= 1u;
+                    }
+                }
+            }
+        } else {
+            const float2 kMagic2 = make_float2(12582912.0f, 12582912.0f), kNegMagic2 = make_float2(-12582912.0f, -12582912.0f);
+            const float2 kNegOne2 = make_float2(-1.0f, -1.0f), kOne2 = make_float2(1.0f, 1.0f);
+            // increments along the two in-plane axes of both rays (packed: .x = ray A, .y = ray B)
+            const float2 rs2 = make_float2((float)RA.rt_a, (float)RB.rt_a), rf2 = make_float2((float)RA.rt_b, (float)RB.rt_b);
+            float2 acc = make_float2(0.0f, 0.0f);
+            int st = 0;
+            unsigned ph = 0;                                             // parity of the full phase to wait for
+            for (int s0 = lo; s0 <= hi; s0 += kSegment) {
+                const int s1 = min(s0 + kSegment - 1, hi), ic = (s0 + s1) >> 1;
+                // fp64 anchors at the segment's middle slice, split into integer voxel index + fraction
+                const double paA = p_of_i(RA.s_a, RA.s_m, RA.rt_a, ic), pbA = p_of_i(RA.s_b, RA.s_m, RA.rt_b, ic);
+                const double paB = p_of_i(RB.s_a, RB.s_m, RB.rt_a, ic), pbB = p_of_i(RB.s_b, RB.s_m, RB.rt_b, ic);
+                const double faA = floor(paA), fbA = floor(pbA), faB = floor(paB), fbB = floor(pbB);
+                const float2 as2 = make_float2((float)(paA - faA), (float)(paB - faB));
+                const float2 af2 = make_float2((float)(pbA - fbA), (float)(pbB - fbB));
+                // per-ray address constant: (integer anchor row) * pitch + (integer anchor column) * 4
+                const unsigned kA = (unsigned)__double2int_rd(faA) * pitchB + ((unsigned)__double2int_rd(fbA) << 2);
+                const unsigned kB = (unsigned)__double2int_rd(faB) * pitchB + ((unsigned)__double2int_rd(fbB) << 2);
+                float2 fi = make_float2((float)(s0 - ic), (float)(s0 - ic));
+                for (int i = s0; i <= s1; ++i) {
+                    tm_mbar_wait(&S.full[st], ph);
+                    const unsigned org = S.org[st];
+                    const float2 ps = __ffma2_rn(fi, rs2, as2), pf = __ffma2_rn(fi, rf2, af2);
+                    fi = __fadd2_rn(fi, kOne2);
+                    const float2 xs = __fadd2_rd(ps, kMagic2), xf = __fadd2_rd(pf, kMagic2);     // bits = 0x4B400000 + floor
+                    const float2 ds = __ffma2_rn(__fadd2_rn(xs, kNegMagic2), kNegOne2, ps);
+                    const float2 df = __ffma2_rn(__fadd2_rn(xf, kNegMagic2), kNegOne2, pf);
+                    const unsigned a0 = __float_as_uint(xs.x) * pitchB + (__float_as_uint(xf.x) << 2) + (kA + org);
+                    const unsigned b0 = __float_as_uint(xs.y) * pitchB + (__float_as_uint(xf.y) << 2) + (kB + org);
+                    const float2 v00 = make_float2(al_lds(a0), al_lds(b0));
+                    const float2 v01 = make_float2(al_lds(a0 + 4u), al_lds(b0 + 4u));
+                    const unsigned a1 = a0 + pitchB, b1 = b0 + pitchB;
+                    const float2 v10 = make_float2(al_lds(a1), al_lds(b1));
+                    const float2 v11 = make_float2(al_lds(a1 + 4u), al_lds(b1 + 4u));
+                    const float2 wf = make_float2(ceil_weight<INTERP>(df.x), ceil_weight<INTERP>(df.y));
+                    const float2 ws = make_float2(ceil_weight<INTERP>(ds.x), ceil_weight<INTERP>(ds.y));
+                    const float2 t0 = __ffma2_rn(wf, __ffma2_rn(v00, kNegOne2, v01), v00);       // row j
+                    const float2 t1 = __ffma2_rn(wf, __ffma2_rn(v10, kNegOne2, v11), v10);       // row j + 1
+                    acc = __fadd2_rn(acc, __ffma2_rn(ws, __ffma2_rn(t0, kNegOne2, t1), t0));
+                    // release the stage: the reads above went through the generic proxy, the next copy into the stage
+                    // comes through the async proxy -- order the two (without this fence the TMA engine was observed
+                    // overwriting words that were still being read: a few wrong rays per projection, not reproducible)
+                    tm_fence_proxy_async();
+                    __syncwarp();
+                    if (lane == 0) tm_mbar_arrive(&S.empty[st]);
+                    if (++st == nst) {
+                        st = 0;
+                        ph ^= 1u;
+                    }
+                }
+            }
+            // a ray that misses the volume (or the degenerate ray) writes +0.0
+            const float oA = RA.i_last >= RA.i_first ? (float)(P.G.delta * RA.L) * acc.x : 0.0f;
+            const float oB = RB.i_last >= RB.i_first ? (float)(P.G.delta * RB.L) * acc.y : 0.0f;
+            if (liveA) P.out[((size_t)proj * P.nv + ivA) * P.nu + iuA] = oA;
+            if (liveB) P.out[((size_t)proj * P.nv + ivB) * P.nu + iuB] = oB;
+            if (liveA) n_samples += max(RA.i_last - RA.i_first + 1, 0);
+            if (liveB) n_samples += max(RB.i_last - RB.i_first + 1, 0);
+        }
+    }
+    if (P.sample_count) block_count_samples(P.sample_count, n_samples);
+}
+
+constexpr size_t tile_smem_bytes() { return kTlTileBytes + sizeof(TlShared); }
+
+}  // namespace fpk

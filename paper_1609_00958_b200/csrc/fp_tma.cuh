@@ -104,6 +104,13 @@ __device__ __forceinline__ void tm_mbar_wait(unsigned long long *bar, unsigned p
         "r"(parity), "r"(0x989680u)
         : "memory");
 }
+// Orders this thread's earlier generic-proxy accesses to shared memory (the tap loads) before later async-proxy
+// accesses (the TMA engine's next write into the same stage) -- issued by every consumer thread before its warp
+// releases a stage.
+__device__ __forceinline__ void tm_fence_proxy_async()
+{
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+}
 __device__ __forceinline__ void tm_load_3d(const CUtensorMap *map, unsigned dst, unsigned long long *bar, int c0, int c1, int c2)
 {
     asm volatile(
@@ -407,6 +414,7 @@ fp_tma_kernel(const __grid_constant__ TmaParams P)
                         const float2 t1 = __ffma2_rn(wz, __ffma2_rn(v10, kNegOne2, v11), v10);   // row j + 1
                         acc[c] = __fadd2_rn(acc[c], __ffma2_rn(make_float2(uy, uy), __ffma2_rn(t0, kNegOne2, t1), t0));
                     }
+                    tm_fence_proxy_async();                        // generic-proxy reads before the next async-proxy write
                     __syncwarp();
                     if (lane == 0) tm_mbar_arrive(&S.empty[s]);
                 }

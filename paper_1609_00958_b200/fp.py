@@ -20,7 +20,7 @@ STATUS = {0: "FP_OK", 1: "FP_ERR_INVALID_ARG", 2: "FP_ERR_CUDA", 3: "FP_ERR_OOM"
 
 OPT_KERNEL, OPT_VOLATILE, OPT_INTERP, OPT_PERMUTED_COPY, OPT_COUNT_SAMPLES, OPT_FOV_CYLINDER, OPT_GROUP = 1, 2, 3, 4, 5, 6, 7
 OPT_TEST_FORCE_TMA = 100
-KERNEL_AUTO, KERNEL_DIRECT, KERNEL_ALIGNED, KERNEL_TMA, KERNEL_TEX, KERNEL_HWLIN = 0, 1, 2, 3, 4, 5
+KERNEL_AUTO, KERNEL_DIRECT, KERNEL_ALIGNED, KERNEL_TMA, KERNEL_TEX, KERNEL_HWLIN, KERNEL_TILE = 0, 1, 2, 3, 4, 5, 6
 INTERP_LINEAR, INTERP_SPLINE = 0, 1
 
 # every symbol include/fp.h declares (tests check the library exports all of them)

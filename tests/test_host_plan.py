@@ -33,15 +33,20 @@ def test_circular_orbits_take_the_aligned_kernel(name, wmax):
         assert 16 <= max(ws) <= wmax, (name, max(ws))
 
 
-def test_general_poses_take_the_direct_kernel_and_report_z_driven_rays():
+def test_general_poses_take_the_tile_kernel_and_report_z_driven_rays():
     cfg = synth.CONFIGS["C4"]
     geom = synth.make_geometry(cfg)
     zs = 0
     with fp.Projector(*cfg.n, cfg.voxel_size, cfg.origin) as P:
         for p in range(cfg.n_proj):
             k, w, z = P.plan(geom[p], cfg.nu, cfg.nv)
-            assert k == fp.KERNEL_DIRECT and w == 0
+            assert k == fp.KERNEL_TILE and w == 0
             zs += z
+        P.set_option(fp.OPT_KERNEL, fp.KERNEL_DIRECT)
+        assert P.plan(geom[0], cfg.nu, cfg.nv)[0] == fp.KERNEL_DIRECT
+    # a volume whose z rows are not a multiple of 4 voxels cannot be addressed by tensor maps: direct kernel
+    with fp.Projector(30, 30, 30, 1.0, (-14.5, -14.5, -14.5)) as P:
+        assert P.plan(geom[0], cfg.nu, cfg.nv)[0] == fp.KERNEL_DIRECT
     # ~70 degree cone: almost every pose has some z-driven rays, a few (source near the xy plane) have none
     assert 0.9 * cfg.n_proj < zs < cfg.n_proj
 
@@ -57,11 +62,11 @@ def test_aligned_kernel_is_refused_when_its_preconditions_fail():
         # a rolled detector: u picks up a z component
         r = g.copy()
         r[6:9] = 0.999 * g[6:9] + 0.04 * g[9:12]
-        assert P.plan(r, cfg.nu, cfg.nv)[0] == fp.KERNEL_DIRECT
+        assert P.plan(r, cfg.nu, cfg.nv)[0] == fp.KERNEL_TILE
         # a tilted rotation axis: v picks up an x component
         t = g.copy()
         t[9] = 1e-9
-        assert P.plan(t, cfg.nu, cfg.nv)[0] == fp.KERNEL_DIRECT
+        assert P.plan(t, cfg.nu, cfg.nv)[0] == fp.KERNEL_TILE
         # a tall detector close to the source: the outer rows are z-driven
         tall = circular_pose(0.3, 100.0, 120.0, 64, 512, 1.5)
         k, w, z = P.plan(tall, 64, 512)
