@@ -389,7 +389,14 @@ fp_tma_kernel(const __grid_constant__ TmaParams P)
                 }
 #pragma unroll
                 for (int s = 0; s < kTmSB; ++s) {
-                    if (s) tm_mbar_wait(&S.full[s], par);
+                    if (s) {
+                        tm_mbar_wait(&S.full[s], par);
+                        // release the PREVIOUS stage here, where its loads have long returned: the proxy fence (generic
+                        // reads before the next async-proxy write into the stage) then has nothing to wait for
+                        tm_fence_proxy_async();
+                        __syncwarp();
+                        if (lane == 0) tm_mbar_arrive(&S.empty[s - 1]);
+                    }
                     const float2 fs = make_float2((float)s, (float)s);
                     uint4 pq2 = make_uint4(0u, 0u, 0u, 0u);
 #pragma unroll
@@ -414,9 +421,11 @@ fp_tma_kernel(const __grid_constant__ TmaParams P)
                         const float2 t1 = __ffma2_rn(wz, __ffma2_rn(v10, kNegOne2, v11), v10);   // row j + 1
                         acc[c] = __fadd2_rn(acc[c], __ffma2_rn(make_float2(uy, uy), __ffma2_rn(t0, kNegOne2, t1), t0));
                     }
-                    tm_fence_proxy_async();                        // generic-proxy reads before the next async-proxy write
-                    __syncwarp();
-                    if (lane == 0) tm_mbar_arrive(&S.empty[s]);
+                    if (s == kTmSB - 1) {
+                        tm_fence_proxy_async();
+                        __syncwarp();
+                        if (lane == 0) tm_mbar_arrive(&S.empty[s]);
+                    }
                 }
             }
         }
