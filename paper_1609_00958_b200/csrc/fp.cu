@@ -47,7 +47,7 @@ struct fp_ctx {
     CUtensorMap tmap[2][kTmWBoxes][kTmMaps];
     const float *tmap_vol = nullptr;
     // tensor maps of the tile kernel: [driving axis][box size]; axis 2 covers the y-fastest copy
-    CUtensorMap tlmap[3][kTlSizes];
+    CUtensorMap tlmap[3][kTlSizes][kTlSizes];
     const float *tlmap_vol = nullptr, *tlmap_perm = nullptr;
     // layout stage of fp_tex_kernel: one layered 2-D array per driving axis (layer = slice), its surface (fill
     // kernel) and two texture objects over it (point sampling for tld4, linear filtering for GJP_hwlin)
@@ -455,10 +455,10 @@ static fp_status build_tile_maps(fp_ctx *c, const float *vol, const float *perm)
         const cuuint64_t nx = c->G.n[0], ny = c->G.n[1], nz = c->G.n[2];
         const cuuint64_t dims[3] = {m == 2 ? ny : nz, m == 2 ? nx : ny, m == 2 ? nz : nx};
         const cuuint64_t strides[2] = {dims[0] * 4, dims[0] * dims[1] * 4};
-        for (int k = 0; k < kTlSizes; ++k) {
-            const cuuint32_t rows = (cuuint32_t)tl_rows(k), cols = (cuuint32_t)tl_cols(k);
+        for (int k = 0; k < kTlSizes * kTlSizes; ++k) {
+            const cuuint32_t rows = (cuuint32_t)tl_rows(k / kTlSizes), cols = (cuuint32_t)tl_cols(k % kTlSizes);
             const cuuint32_t box[3] = {cols, m == 1 ? 1u : rows, m == 1 ? rows : 1u};
-            const CUresult r = g_encode(&c->tlmap[m][k], CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, (void *)(m == 2 ? perm : vol), dims,
+            const CUresult r = g_encode(&c->tlmap[m][k / kTlSizes][k % kTlSizes], CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, (void *)(m == 2 ? perm : vol), dims,
                                         strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
                                         CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
             if (r != CUDA_SUCCESS) {

@@ -31,16 +31,16 @@ namespace fpk {
 constexpr int kTlU = 32, kTlV = 16;              // detector pixels per block along u and v
 constexpr int kTlConsumers = kTlU * kTlV / 2;    // two rays per consumer thread
 constexpr int kTlThreads = kTlConsumers + 32;    // + one producer warp
-constexpr int kTlSizes = 3;                      // box sizes (rows x cols); cols % 32 = 4 or 20 words: rows fall in different banks
-__host__ __device__ constexpr int tl_rows(int k) { return k == 0 ? 28 : (k == 1 ? 44 : 60); }
-__host__ __device__ constexpr int tl_cols(int k) { return k == 0 ? 36 : (k == 1 ? 52 : 68); }
-constexpr int kTlStagesMax = 4;                  // four stages of the two smaller boxes, three of the largest
-// stage strides are multiples of 128 B (TMA destination alignment): 9216 >= 44 x 52 x 4, 16384 >= 60 x 68 x 4
-__host__ __device__ constexpr unsigned tl_stage_stride(int k) { return k == 2 ? 16384u : 9216u; }
-constexpr unsigned kTlTileBytes = 3u * 16384u;   // = 49152 >= 4 x 9216
+constexpr int kTlSizes = 5;                      // box classes per dimension: a block takes the smallest rows x cols box that holds its quadrilaterals
+__host__ __device__ constexpr int tl_rows(int k) { return k == 0 ? 20 : (k == 1 ? 28 : (k == 2 ? 36 : (k == 3 ? 44 : 60))); }
+__host__ __device__ constexpr int tl_cols(int k) { return k == 0 ? 28 : (k == 1 ? 36 : (k == 2 ? 44 : (k == 3 ? 52 : 68))); }
+constexpr int kTlStagesMax = 12;                 // slices in flight: as many stages as fit the 48 KB of tiles, at most 12
+constexpr unsigned kTlTileBytes = 49152u;
+// a stage is the box rounded up to 128 B (TMA destination alignment)
+__host__ __device__ constexpr unsigned tl_stage_stride(int rows, int cols) { return ((unsigned)(rows * cols * 4) + 127u) & ~127u; }
 
 struct __align__(64) TileParams {
-    CUtensorMap map[3][kTlSizes];      // [driving axis][box size]
+    CUtensorMap map[3][kTlSizes][kTlSizes];   // [driving axis][rows class][cols class]
     GridDesc G;
     AxisLayout lay[3];                 // for the direct path of tiles that do not qualify
     const ProjDesc *proj;              // all projections of the call
@@ -61,7 +61,7 @@ struct __align__(16) TlShared {
     TlCorner corner[4];
     int m[4];                          // driving axis (+ 4 if r_m < 0) of the corner rays; -1: degenerate
     int lo, hi;                        // slice range of the block (union of its rays' ranges)
-    int size, staged;                  // box size index; 1: staged path, 0: direct path
+    int size_r, size_c, staged;        // box classes; staged = 1: staged path, 0: direct path
 };
 
 // Direct path for one ray (the body of fp_direct_kernel).
@@ -165,7 +165,7 @@ fp_tile_kernel(const __grid_constant__ TileParams P)
     // ---- does the tile qualify for the staged path?  Box of the corner quadrilateral at both ends of the slice range
     //      (every corner point is affine in the slice index, so the extents are largest at one of the ends)
     if (tid == 0) {
-        int size = -1;
+        int size_r = -1, size_c = -1;
         if (same_m && S.hi >= S.lo) {
             int rows = 0, cols = 0;
             for (int e = 0; e < 2; ++e) {
@@ -182,11 +182,14 @@ fp_tile_kernel(const __grid_constant__ TileParams P)
                 rows = max(rows, (int)fmin(smax - smin, 1.0e6) + 5);
                 cols = max(cols, (int)fmin(fmax_ - fmin_, 1.0e6) + 8);     // + 3: the box starts on a 16-byte boundary
             }
-            for (int k = kTlSizes - 1; k >= 0; --k)
-                if (rows <= tl_rows(k) && cols <= tl_cols(k)) size = k;
+            for (int k = kTlSizes - 1; k >= 0; --k) {
+                if (rows <= tl_rows(k)) size_r = k;
+                if (cols <= tl_cols(k)) size_c = k;
+            }
         }
-        S.size = max(size, 0);
-        S.staged = size >= 0;
+        S.size_r = max(size_r, 0);
+        S.size_c = max(size_c, 0);
+        S.staged = size_r >= 0 && size_c >= 0;
     }
     __syncthreads();
 
@@ -201,17 +204,17 @@ fp_tile_kernel(const __grid_constant__ TileParams P)
             if (liveB) n_samples += max(RB.i_last - RB.i_first + 1, 0);
         }
     } else {
-        const int lo = S.lo, hi = S.hi, size = S.size;
+        const int lo = S.lo, hi = S.hi;
         const int n_slices = hi - lo + 1;
-        const int nst = size == 2 ? 3 : 4;                               // stages in flight
-        const int rows = tl_rows(size), cols = tl_cols(size);
-        const unsigned pitchB = (unsigned)cols * 4u, boxB = (unsigned)(rows * cols * 4), stageB = tl_stage_stride(size);
+        const int rows = tl_rows(S.size_r), cols = tl_cols(S.size_c);
+        const unsigned pitchB = (unsigned)cols * 4u, boxB = (unsigned)(rows * cols * 4), stageB = tl_stage_stride(rows, cols);
+        const int nst = min(kTlStagesMax, (int)(kTlTileBytes / stageB));   // stages in flight
         if (producer) {
             // lane = slice-in-batch * 8 + corner * 2 + coordinate; batches of four slices
             const int sb = lane >> 3, cc = (lane >> 1) & 3, co = lane & 1;
             const TlCorner C = S.corner[cc];
             const double s_t = co ? C.s_b : C.s_a, rt_t = co ? C.rt_b : C.rt_a;
-            const CUtensorMap *map = &P.map[m_tile][size];
+            const CUtensorMap *map = &P.map[m_tile][S.size_r][S.size_c];
             int st = 0;
             unsigned ph = 0;                                             // parity of the empty phase to wait for (from the second round on)
             for (int n0 = 0; n0 < n_slices; n0 += 4) {
