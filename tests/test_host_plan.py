@@ -70,7 +70,7 @@ def test_aligned_kernel_is_refused_when_its_preconditions_fail():
         # a tall detector close to the source: the outer rows are z-driven
         tall = circular_pose(0.3, 100.0, 120.0, 64, 512, 1.5)
         k, w, z = P.plan(tall, 64, 512)
-        assert k == fp.KERNEL_DIRECT and z
+        assert k == fp.KERNEL_TILE and z
         # the forced direct kernel
         P.set_option(fp.OPT_KERNEL, fp.KERNEL_DIRECT)
         assert P.plan(g, cfg.nu, cfg.nv)[0] == fp.KERNEL_DIRECT
@@ -84,7 +84,7 @@ def test_window_grows_with_the_row_spacing():
     with fp.Projector(*cfg.n, cfg.voxel_size, cfg.origin) as P:
         w1 = P.plan(circular_pose(0.1, cfg.sid, cfg.sdd, 768, 768, 1.0), 768, 768)[1]
         w2 = P.plan(circular_pose(0.1, cfg.sid, cfg.sdd, 768, 768, 1.6), 768, 768)[1]
-        # a detector too coarse for the largest window falls back to the direct kernel
+        # a detector too coarse for the largest window falls back to the general-pose (tile) kernel
         k3, w3, _ = P.plan(circular_pose(0.1, cfg.sid, cfg.sdd, 768, 768, 4.0), 768, 768)
     assert 0 < w1 < w2 <= 512
-    assert k3 == fp.KERNEL_DIRECT and w3 == 0
+    assert k3 == fp.KERNEL_TILE and w3 == 0
