@@ -169,7 +169,8 @@ fp_status fp_project_host(fp_ctx *ctx, const float *vol_host, int n_proj, const 
  * iterative reconstruction pairs the projector with its back-projection).  With A the linear map
  * volume -> projections that fp_project computes for these poses, writes vol_out = A^T proj: every tap of
  * every sample of every ray receives voxel_size * ||r~|| * w * w * proj[ray] (same set-up, slices, taps and
- * weights; FP_OPT_INTERP applies).  fp32 reductions in arbitrary order: results are reproducible only to
+ * weights; FP_OPT_INTERP applies).  fp32 reductions (RED.ADD.F32.FTZ: denormal contributions are flushed to
+ * zero) in arbitrary order: results are reproducible only to
  * fp32 rounding of the sum.
  *   proj_dev     device, fp32 [n_proj][nv][nu]
  *   vol_out_dev  device, fp32 [nx][ny][nz], fully overwritten (cleared first, also for n_proj = 0)
