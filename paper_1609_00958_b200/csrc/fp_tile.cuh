@@ -257,7 +257,7 @@ fp_tile_kernel(const __grid_constant__ TileParams P)
             // increments along the two in-plane axes of both rays (packed: .x = ray A, .y = ray B)
             const float2 rs2 = make_float2((float)RA.rt_a, (float)RB.rt_a), rf2 = make_float2((float)RA.rt_b, (float)RB.rt_b);
             float2 acc = make_float2(0.0f, 0.0f);
-            int st = 0;
+            int st = 0, prev = -1;
             unsigned ph = 0;                                             // parity of the full phase to wait for
             for (int s0 = lo; s0 <= hi; s0 += kSegment) {
                 const int s1 = min(s0 + kSegment - 1, hi), ic = (s0 + s1) >> 1;
@@ -273,6 +273,16 @@ fp_tile_kernel(const __grid_constant__ TileParams P)
                 float2 fi = make_float2((float)(s0 - ic), (float)(s0 - ic));
                 for (int i = s0; i <= s1; ++i) {
                     tm_mbar_wait(&S.full[st], ph);
+                    // release the PREVIOUS stage here, where its loads have returned.  The reads went through the
+                    // generic proxy, the next copy into the stage comes through the async proxy: the fence orders
+                    // the two (without it the TMA engine was observed overwriting words that were still being read:
+                    // a few wrong rays per projection, not reproducible)
+                    if (prev >= 0) {
+                        tm_fence_proxy_async();
+                        __syncwarp();
+                        if (lane == 0) tm_mbar_arrive(&S.empty[prev]);
+                    }
+                    prev = st;
                     const unsigned org = S.org[st];
                     const float2 ps = __ffma2_rn(fi, rs2, as2), pf = __ffma2_rn(fi, rf2, af2);
                     fi = __fadd2_rn(fi, kOne2);
@@ -291,12 +301,6 @@ fp_tile_kernel(const __grid_constant__ TileParams P)
                     const float2 t0 = __ffma2_rn(wf, __ffma2_rn(v00, kNegOne2, v01), v00);       // row j
                     const float2 t1 = __ffma2_rn(wf, __ffma2_rn(v10, kNegOne2, v11), v10);       // row j + 1
                     acc = __fadd2_rn(acc, __ffma2_rn(ws, __ffma2_rn(t0, kNegOne2, t1), t0));
-                    // release the stage: the reads above went through the generic proxy, the next copy into the stage
-                    // comes through the async proxy -- order the two (without this fence the TMA engine was observed
-                    // overwriting words that were still being read: a few wrong rays per projection, not reproducible)
-                    tm_fence_proxy_async();
-                    __syncwarp();
-                    if (lane == 0) tm_mbar_arrive(&S.empty[st]);
                     if (++st == nst) {
                         st = 0;
                         ph ^= 1u;
