@@ -314,7 +314,8 @@ static int plan_lane_v(const double *g, int nu, int nv, bool permuted)
 // 16-byte aligned volume (float4 loads along z).  The window bound is conservative: the largest
 // ray parameter |t| = |(i - s_m) / r_m| over all slices a batch can touch, times the r_z spread
 // of the rows of one block, plus the drift inside a batch, alignment and tap margins.
-static int plan_aligned(const fp_ctx *c, const float *vol, const double *g, int nu, int nv, int *tile_rows = nullptr)
+static int plan_aligned(const fp_ctx *c, const float *vol, const double *g, int nu, int nv, int *tile_rows = nullptr,
+                        int block_rows = kAlTV)
 {
     if (tile_rows) *tile_rows = 1 << 30;
     for (int k = 0; k < 12; ++k)
@@ -357,7 +358,7 @@ static int plan_aligned(const fp_ctx *c, const float *vol, const double *g, int 
     if (!(rz_max <= rm_min * (1.0 - 1e-9))) return 0;            // a z-driven (or tied) ray somewhere
     if (!(t_lo <= t_hi)) return 16;                              // every column misses: any window will do
     const double t_max = std::max(std::fabs(t_lo), std::fabs(t_hi));
-    const int rows = std::min(nv, kAlTV);
+    const int rows = std::min(nv, block_rows);
     // rows of one block at one t, the drift inside a batch, and the difference in t between the columns
     // of a block, which share one window: their first slices differ (entry through a side face) and
     // their r_m differ by at most kAlTU detector steps
@@ -395,7 +396,7 @@ static fp_status ensure_ids(fp_ctx *c, int n_proj)
         c->ids_cap = 0;
     }
     const int cap = n_proj + 64;
-    FP_CUDA(c, cudaMalloc(&c->ids_dev, sizeof(int) * 4 * (size_t)cap));
+    FP_CUDA(c, cudaMalloc(&c->ids_dev, sizeof(int) * 5 * (size_t)cap));
     c->ids_cap = cap;
     return FP_OK;
 }
@@ -500,19 +501,34 @@ static fp_status build_tensor_maps(fp_ctx *c, const float *vol)
     return FP_OK;
 }
 
-template <int INTERP>
+// Does a pose with this z window and these volume rows per slice fit fp_tma_kernel's tiles?
+static bool fits_tma(int window, int rows) { return window > 0 && window <= kTmW && rows <= kTmNR; }
+
+template <int INTERP, int ROWS>
 static fp_status launch_tma(fp_ctx *c, const TmaParams &T, dim3 grid, cudaStream_t st)
 {
     // per device and cheap: set on every launch
     const size_t smem = tma_smem_bytes();
-    FP_CUDA(c, cudaFuncSetAttribute(fp_tma_kernel<INTERP>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    fp_tma_kernel<INTERP><<<grid, kTmThreads, smem, st>>>(T);
+    FP_CUDA(c, cudaFuncSetAttribute(fp_tma_kernel<INTERP, ROWS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    fp_tma_kernel<INTERP, ROWS><<<grid, tm_threads(ROWS), smem, st>>>(T);
     FP_CUDA(c, cudaGetLastError());
     return FP_OK;
 }
 
-// Does a pose with this z window and these volume rows per slice fit fp_tma_kernel's tiles?
-static bool fits_tma(int window, int rows) { return window > 0 && window <= kTmW && rows <= kTmNR; }
+// Which fp_tma_kernel takes an aligned pose: 256 detector rows per block, 192 where only their narrower z window
+// fits the largest TMA box, 0 = neither.  w256 / tile_rows: plan_aligned() of the pose for 256-row blocks.
+static int tma_block_rows(const fp_ctx *c, const float *vol, const double *g, int nu, int nv, int w256, int tile_rows,
+                          int *window = nullptr)
+{
+    if (window) *window = w256;
+    if (fits_tma(w256, tile_rows)) return kTmRows;
+    if (w256 <= 0 || tile_rows > kTmNR) return 0;
+    const int w = plan_aligned(c, vol, g, nu, nv, nullptr, kTmRowsNarrow);
+    if (!fits_tma(w, tile_rows)) return 0;
+    if (window) *window = w;
+    return kTmRowsNarrow;
+}
+
 
 // Layout stage of fp_tex_kernel (sec. 2.8): the layered array of driving axis `axis`
 // (layer = slice, row = slow transverse axis, column = fast transverse axis), filled from the caller's volume
@@ -678,7 +694,7 @@ extern "C" fp_status fp_project(fp_ctx *c, const float *vol_dev, int n_proj, con
     if (s != FP_OK) return s;
 
     // plan: which kernel takes which projection
-    std::vector<int> ids_al, ids_di, ids_tm, ids_tx;
+    std::vector<int> ids_al, ids_di, ids_tm, ids_tn, ids_tx;
     int w_al = 0;
     const bool all_tex = c->opt_kernel == FP_KERNEL_TEX || c->opt_kernel == FP_KERNEL_HWLIN;
     for (int p = 0; p < n_proj; ++p) {
@@ -688,8 +704,13 @@ extern "C" fp_status fp_project(fp_ctx *c, const float *vol_dev, int n_proj, con
         }
         int rows = 0;
         const int w = c->opt_kernel == FP_KERNEL_DIRECT ? 0 : plan_aligned(c, vol_dev, geom + 12 * (size_t)p, nu, nv, &rows);
-        if ((fits_tma(w, rows) || (c->opt_force_tma && w > 0)) && c->opt_kernel != FP_KERNEL_ALIGNED) {
+        const int tm_rows = c->opt_kernel == FP_KERNEL_ALIGNED ? 0
+                            : (c->opt_force_tma && w > 0) ? kTmRows
+                                                          : tma_block_rows(c, vol_dev, geom + 12 * (size_t)p, nu, nv, w, rows);
+        if (tm_rows == kTmRows) {
             ids_tm.push_back(p);                       // fits the TMA-fed kernel's tile
+        } else if (tm_rows == kTmRowsNarrow) {
+            ids_tn.push_back(p);                       // ... with 192 detector rows per block
         } else if (w > 0 && w <= kAlignedMaxW) {
             ids_al.push_back(p);
             w_al = std::max(w_al, w);
@@ -729,6 +750,8 @@ extern "C" fp_status fp_project(fp_ctx *c, const float *vol_dev, int n_proj, con
     if (!ids_tm.empty())
         FP_CUDA(c, cudaMemcpyAsync(c->ids_dev + 2 * c->ids_cap, ids_tm.data(), sizeof(int) * ids_tm.size(),
                                    cudaMemcpyHostToDevice, st));
+    if (!ids_tn.empty())
+        FP_CUDA(c, cudaMemcpyAsync(c->ids_dev + 4 * c->ids_cap, ids_tn.data(), sizeof(int) * ids_tn.size(), cudaMemcpyHostToDevice, st));
     if (!ids_tx.empty())
         FP_CUDA(c, cudaMemcpyAsync(c->ids_dev + 3 * c->ids_cap, ids_tx.data(), sizeof(int) * ids_tx.size(),
                                    cudaMemcpyHostToDevice, st));
@@ -753,27 +776,33 @@ extern "C" fp_status fp_project(fp_ctx *c, const float *vol_dev, int n_proj, con
         if (s != FP_OK) return s;
         c->last_launches += 1;
     }
-    if (!ids_tm.empty()) {
+    for (int narrow = 0; narrow < 2; ++narrow) {
+        const std::vector<int> &ids = narrow ? ids_tn : ids_tm;
+        if (ids.empty()) continue;
+        const int block_rows = narrow ? kTmRowsNarrow : kTmRows;
         s = build_tensor_maps(c, vol_dev);
         if (s != FP_OK) return s;
         TmaParams T;
         memcpy(T.map, c->tmap, sizeof T.map);
         T.G = c->G;
         T.proj = c->proj_dev;
-        T.ids = c->ids_dev + 2 * c->ids_cap;
+        T.ids = c->ids_dev + (narrow ? 4 : 2) * c->ids_cap;
         T.out = out_dev;
         T.sample_count = c->opt_count ? c->count_dev : nullptr;
         T.err_flag = reinterpret_cast<unsigned int *>(c->count_dev + 1);
         T.nu = nu;
         T.nv = nv;
-        T.n_sel = (int)ids_tm.size();
+        T.n_sel = (int)ids.size();
         T.fov = c->opt_fov;
         T.out_vec = ((uintptr_t)out_dev & 15) == 0 && (nu & 3) == 0;
         // groups of neighbouring poses share their volume rows through L2 (fp_tma.cuh)
-        T.group = std::max(1, std::min(c->opt_group, (int)ids_tm.size()));
-        dim3 grid((unsigned)((nu + kTmTU - 1) / kTmTU * T.group), (unsigned)((nv + kTmRows - 1) / kTmRows),
-                  (unsigned)((ids_tm.size() + T.group - 1) / T.group));
-        s = c->opt_interp == FP_INTERP_SPLINE ? launch_tma<1>(c, T, grid, st) : launch_tma<0>(c, T, grid, st);
+        T.group = std::max(1, std::min(c->opt_group, (int)ids.size()));
+        dim3 grid((unsigned)((nu + kTmTU - 1) / kTmTU * T.group), (unsigned)((nv + block_rows - 1) / block_rows),
+                  (unsigned)((ids.size() + T.group - 1) / T.group));
+        if (narrow)
+            s = c->opt_interp == FP_INTERP_SPLINE ? launch_tma<1, kTmRowsNarrow>(c, T, grid, st) : launch_tma<0, kTmRowsNarrow>(c, T, grid, st);
+        else
+            s = c->opt_interp == FP_INTERP_SPLINE ? launch_tma<1, kTmRows>(c, T, grid, st) : launch_tma<0, kTmRows>(c, T, grid, st);
         if (s != FP_OK) return s;
         c->last_launches += 1;
     }
@@ -938,8 +967,9 @@ extern "C" fp_status fp_plan(fp_ctx *c, const double *geom, int nu, int nv, int 
     const int w = c->opt_kernel == FP_KERNEL_DIRECT ? 0 : plan_aligned(c, nullptr, geom, nu, nv, &rows);
     const bool al = w > 0 && w <= kAlignedMaxW;
     *kernel = al ? FP_KERNEL_ALIGNED : ((c->opt_kernel != FP_KERNEL_DIRECT && (c->G.n[2] & 3) == 0) ? FP_KERNEL_TILE : FP_KERNEL_DIRECT);
-    if (al && c->opt_kernel != FP_KERNEL_ALIGNED && fits_tma(w, rows)) *kernel = FP_KERNEL_TMA;
     *window = al ? w : 0;
+    // the TMA-fed kernel reports the window of its own blocks (256 or 192 detector rows)
+    if (al && c->opt_kernel != FP_KERNEL_ALIGNED && tma_block_rows(c, nullptr, geom, nu, nv, w, rows, window) != 0) *kernel = FP_KERNEL_TMA;
     if (c->opt_kernel == FP_KERNEL_TEX || c->opt_kernel == FP_KERNEL_HWLIN) {
         *kernel = c->opt_kernel;                           // every pose goes through the texture pipe
         *window = 0;

@@ -28,9 +28,9 @@ namespace fpk {
 
 constexpr int kTmTU = 8;                 // detector columns per block
 constexpr int kTmSB = 4;                 // slices per batch = pipeline stages
-constexpr int kTmRows = 256;             // detector rows per block, two per consumer thread
-constexpr int kTmConsumers = kTmRows / 2;
-constexpr int kTmThreads = kTmConsumers + 32;
+constexpr int kTmRows = 256;             // detector rows per block, two per consumer thread ...
+constexpr int kTmRowsNarrow = 192;       // ... or 192 where the z window of 256 rows does not fit the largest box (wide cones)
+__host__ __device__ constexpr int tm_threads(int rows) { return rows / 2 + 32; }   // consumers + one producer warp
 constexpr int kTmW = 256;                // largest z window (voxels) = largest inner TMA box size
 constexpr int kTmWBoxes = 4;             // inner box sizes 160, 192, 224, 256: the tile's row pitch follows the box
 constexpr int kTmWMin = 160, kTmWStep = 32;
@@ -256,6 +256,7 @@ __device__ __forceinline__ void tm_produce_batch(TmShared &S, const TmaParams &P
         if (s == ss) S.stage_col[ss][c] = make_uint2(addr0, wbits);
         __syncwarp();
         if (lane == 0) {
+            tm_fence_proxy_async();
             if (bytes) {
                 tm_mbar_arrive_tx(&S.full[ss], bytes);
                 const CUtensorMap *map = &P.map[pass][wi][mi_s];
@@ -285,10 +286,12 @@ __device__ __forceinline__ float tm_step_length(const TmShared &S, const TmaPara
     return (float)(P.G.delta * L);
 }
 
-template <int INTERP>
-__global__ void __launch_bounds__(kTmThreads, 4)
+template <int INTERP, int ROWS>
+__global__ void __launch_bounds__(tm_threads(ROWS), 4)
 fp_tma_kernel(const __grid_constant__ TmaParams P)
 {
+    constexpr int kTmConsumers = ROWS / 2;
+    static_assert(ROWS % 64 == 0 && ROWS <= 256, "whole consumer warps of two rows per thread");
     extern __shared__ __align__(128) unsigned char tm_smem_raw[];
     float *tiles = reinterpret_cast<float *>(tm_smem_raw);                   // kTmSB stages, then the zero region; 128-byte aligned
     TmShared &S = *reinterpret_cast<TmShared *>(tm_smem_raw + kTmTileBytes + sizeof(float) * kTmZeroFloats);
@@ -303,8 +306,8 @@ fp_tma_kernel(const __grid_constant__ TmaParams P)
     const int proj = P.ids[sel];
     const double *g = P.proj[proj].g;
     const int iu0 = (int)(blockIdx.x / (unsigned)P.group) * kTmTU;
-    const int row0 = blockIdx.y * kTmRows;
-    // consumer thread t carries detector rows row0 + t and row0 + 128 + t
+    const int row0 = blockIdx.y * ROWS;
+    // consumer thread t carries detector rows row0 + t and row0 + ROWS / 2 + t
     const int ct = min(tid, kTmConsumers - 1);
     const int iv0 = min(row0 + ct, P.nv - 1), iv1 = min(row0 + kTmConsumers + ct, P.nv - 1);
 
@@ -325,7 +328,7 @@ fp_tma_kernel(const __grid_constant__ TmaParams P)
             S.s[1] = s[1];
             S.s[2] = s[2];
             S.rho_first = al_rho(g, P.G, row0, s[2]);
-            S.rho_last = al_rho(g, P.G, min(row0 + kTmRows, P.nv) - 1, s[2]);
+            S.rho_last = al_rho(g, P.G, min(row0 + ROWS, P.nv) - 1, s[2]);
 #pragma unroll
             for (int k = 0; k < kTmSB; ++k) {
                 tm_mbar_init(&S.full[k], 1);
@@ -393,7 +396,6 @@ fp_tma_kernel(const __grid_constant__ TmaParams P)
                         tm_mbar_wait(&S.full[s], par);
                         // release the PREVIOUS stage here, where its loads have long returned: the proxy fence (generic
                         // reads before the next async-proxy write into the stage) then has nothing to wait for
-                        tm_fence_proxy_async();
                         __syncwarp();
                         if (lane == 0) tm_mbar_arrive(&S.empty[s - 1]);
                     }
@@ -422,7 +424,6 @@ fp_tma_kernel(const __grid_constant__ TmaParams P)
                         acc[c] = __fadd2_rn(acc[c], __ffma2_rn(make_float2(uy, uy), __ffma2_rn(t0, kNegOne2, t1), t0));
                     }
                     if (s == kTmSB - 1) {
-                        tm_fence_proxy_async();
                         __syncwarp();
                         if (lane == 0) tm_mbar_arrive(&S.empty[s]);
                     }
