@@ -16,9 +16,14 @@
 // outside its own slice range [i_first, i_last] has a transverse coordinate outside (-1, N_t), so all its taps
 // lie in the zero fill: no masks, no per-ray loop bounds.
 //
+// Three blocks per SM (72 registers): the fp64 parameters of a thread's two rays are parked in shared memory
+// during the loop (read back once per segment), and the loop walks the barrier / origin arrays with one running
+// byte address, so its stage bookkeeping runs on the uniform datapath (45 instructions per warp and slice).
+//
 // Tiles whose corner rays have different driving axes (about 4 % of C4's tiles), whose box would not fit the
 // largest stage, or whose rays all miss run the direct path (fp_kernels.cuh) inside the same launch.
 #pragma once
+#include <cstddef>
 #include <cstdint>
 #include <cuda.h>
 #include <cuda_runtime.h>
@@ -56,13 +61,42 @@ struct TlCorner {                      // one corner ray, parametrised along the
 };
 
 struct __align__(16) TlShared {
+    // the consumers walk these three arrays with ONE running byte address (stage * 8): keep them 8 bytes per stage
+    // and in this order (kTlEmptyOff, kTlOrgOff below)
     unsigned long long full[kTlStagesMax], empty[kTlStagesMax];
-    unsigned org[kTlStagesMax];        // per stage: byte address of tile word (0, 0) minus (js0 * pitch + kf0) * 4 terms, see below
+    uint2 org[kTlStagesMax];           // .x per stage: byte address of tile word (0, 0) minus (js0 * pitch + kf0) * 4 terms, see below
+    unsigned long long sink;           // barrier nobody waits on: takes the release of "the stage before the first"
     TlCorner corner[4];
     int m[4];                          // driving axis (+ 4 if r_m < 0) of the corner rays; -1: degenerate
     int lo, hi;                        // slice range of the block (union of its rays' ranges)
     int size_r, size_c, staged;        // box classes; staged = 1: staged path, 0: direct path
 };
+
+constexpr unsigned kTlEmptyOff = 8u * kTlStagesMax, kTlOrgOff = 16u * kTlStagesMax, kTlSinkOff = 24u * kTlStagesMax;
+static_assert(offsetof(TlShared, empty) == kTlEmptyOff && offsetof(TlShared, org) == kTlOrgOff && offsetof(TlShared, sink) == kTlSinkOff,
+              "TlShared layout");
+// fp64 parameters of the two rays of every consumer thread, parked in shared memory while the sampling loop runs (they
+// are needed once per segment only; in registers they would cost a third of the occupancy): [4][kTlConsumers] double2
+constexpr unsigned kTlRayBytes = 4u * kTlConsumers * 16u;
+
+__device__ __forceinline__ void tl_wait_addr(unsigned bar, unsigned parity)
+{
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "WAIT_%=:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1, %2;\n"
+        "@p bra DONE_%=;\n"
+        "bra WAIT_%=;\n"
+        "DONE_%=:\n"
+        "}\n" ::"r"(bar),
+        "r"(parity), "r"(0x989680u)
+        : "memory");
+}
+__device__ __forceinline__ void tl_arrive_addr(unsigned bar)
+{
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
 
 // Direct path for one ray (the body of fp_direct_kernel).
 template <int INTERP>
@@ -86,7 +120,7 @@ __device__ __forceinline__ float tl_direct_ray(const RaySetup &R, const AxisLayo
 }
 
 template <int INTERP>
-__global__ void __launch_bounds__(kTlThreads, 2)
+__global__ void __launch_bounds__(kTlThreads, 3)
 fp_tile_kernel(const __grid_constant__ TileParams P)
 {
     extern __shared__ __align__(128) unsigned char tl_smem_raw[];
@@ -121,6 +155,7 @@ fp_tile_kernel(const __grid_constant__ TileParams P)
             tm_mbar_init(&S.full[k], 1);
             tm_mbar_init(&S.empty[k], kTlConsumers / 32);
         }
+        tm_mbar_init(&S.sink, kTlConsumers / 32);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncthreads();
@@ -232,8 +267,11 @@ fp_tile_kernel(const __grid_constant__ TileParams P)
                     const int js0 = __shfl_sync(0xffffffffu, js0_l, 8 * q), kf0 = __shfl_sync(0xffffffffu, kf0_l, 8 * q);
                     if (n >= nst) tm_mbar_wait(&S.empty[st], ph);
                     if (lane == 0) {
+                        // the consumers' reads of this stage (generic proxy, ordered before this point by their
+                        // arrival on empty[]) before the copy below (async proxy)
+                        tm_fence_proxy_async();
                         // consumers add bits(row) * pitch + bits(col) * 4 with bits = 0x4B400000 + index (mod 2^32)
-                        S.org[st] = tiles_smem + st * stageB - ((0x4B400000u + (unsigned)js0) * pitchB + ((0x4B400000u + (unsigned)kf0) << 2));
+                        S.org[st].x = tiles_smem + st * stageB - ((0x4B400000u + (unsigned)js0) * pitchB + ((0x4B400000u + (unsigned)kf0) << 2));
                         tm_mbar_arrive_tx(&S.full[st], boxB);
                         const unsigned dst = tiles_smem + st * stageB;
                         const int ii = lo + n;
@@ -254,36 +292,51 @@ fp_tile_kernel(const __grid_constant__ TileParams P)
         } else {
             const float2 kMagic2 = make_float2(12582912.0f, 12582912.0f), kNegMagic2 = make_float2(-12582912.0f, -12582912.0f);
             const float2 kNegOne2 = make_float2(-1.0f, -1.0f), kOne2 = make_float2(1.0f, 1.0f);
-            // increments along the two in-plane axes of both rays (packed: .x = ray A, .y = ray B)
-            const float2 rs2 = make_float2((float)RA.rt_a, (float)RB.rt_a), rf2 = make_float2((float)RA.rt_b, (float)RB.rt_b);
+            // what the loop needs of the two rays: the fp64 parameters go to shared memory (read back once per
+            // segment), the rest is folded into two scales and a count -- RA / RB are dead from here on
+            double2 *rayp = reinterpret_cast<double2 *>(tl_smem_raw + kTlTileBytes + sizeof(TlShared)) + tid;
+            rayp[0 * kTlConsumers] = make_double2(RA.s_a, RA.rt_a);
+            rayp[1 * kTlConsumers] = make_double2(RA.s_b, RA.rt_b);
+            rayp[2 * kTlConsumers] = make_double2(RB.s_a, RB.rt_a);
+            rayp[3 * kTlConsumers] = make_double2(RB.s_b, RB.rt_b);
+            const double s_m = S.corner[0].s_m;                          // the source's coordinate along m: the same for every ray
+            // scale Delta ||r~||; a ray that misses the volume (or the degenerate ray) writes +0.0
+            const float scA = RA.i_last >= RA.i_first ? (float)(P.G.delta * RA.L) : 0.0f;
+            const float scB = RB.i_last >= RB.i_first ? (float)(P.G.delta * RB.L) : 0.0f;
+            if (liveA) n_samples += max(RA.i_last - RA.i_first + 1, 0);
+            if (liveB) n_samples += max(RB.i_last - RB.i_first + 1, 0);
+            const size_t outA = ((size_t)proj * P.nv + ivA) * P.nu + iuA, outB = ((size_t)proj * P.nv + ivB) * P.nu + iuB;
+
             float2 acc = make_float2(0.0f, 0.0f);
-            int st = 0, prev = -1;
+            // one running address walks full[], empty[] (+ kTlEmptyOff) and org[] (+ kTlOrgOff)
+            const unsigned bar0 = tm_smem(&S.full[0]), bar_end = bar0 + 8u * (unsigned)nst;
+            unsigned bar = bar0, prev = bar0 + (kTlSinkOff - kTlEmptyOff);
             unsigned ph = 0;                                             // parity of the full phase to wait for
             for (int s0 = lo; s0 <= hi; s0 += kSegment) {
                 const int s1 = min(s0 + kSegment - 1, hi), ic = (s0 + s1) >> 1;
                 // fp64 anchors at the segment's middle slice, split into integer voxel index + fraction
-                const double paA = p_of_i(RA.s_a, RA.s_m, RA.rt_a, ic), pbA = p_of_i(RA.s_b, RA.s_m, RA.rt_b, ic);
-                const double paB = p_of_i(RB.s_a, RB.s_m, RB.rt_a, ic), pbB = p_of_i(RB.s_b, RB.s_m, RB.rt_b, ic);
+                const double2 qa = rayp[0 * kTlConsumers], qb = rayp[1 * kTlConsumers];
+                const double2 qc = rayp[2 * kTlConsumers], qd = rayp[3 * kTlConsumers];
+                const double paA = p_of_i(qa.x, s_m, qa.y, ic), pbA = p_of_i(qb.x, s_m, qb.y, ic);
+                const double paB = p_of_i(qc.x, s_m, qc.y, ic), pbB = p_of_i(qd.x, s_m, qd.y, ic);
+                // increments along the two in-plane axes of both rays (packed: .x = ray A, .y = ray B)
+                const float2 rs2 = make_float2((float)qa.y, (float)qc.y), rf2 = make_float2((float)qb.y, (float)qd.y);
                 const double faA = floor(paA), fbA = floor(pbA), faB = floor(paB), fbB = floor(pbB);
                 const float2 as2 = make_float2((float)(paA - faA), (float)(paB - faB));
                 const float2 af2 = make_float2((float)(pbA - fbA), (float)(pbB - fbB));
                 // per-ray address constant: (integer anchor row) * pitch + (integer anchor column) * 4
-                const unsigned kA = (unsigned)__double2int_rd(faA) * pitchB + ((unsigned)__double2int_rd(fbA) << 2);
-                const unsigned kB = (unsigned)__double2int_rd(faB) * pitchB + ((unsigned)__double2int_rd(fbB) << 2);
+                unsigned kA = (unsigned)__double2int_rd(faA) * pitchB + ((unsigned)__double2int_rd(fbA) << 2);
+                unsigned kB = (unsigned)__double2int_rd(faB) * pitchB + ((unsigned)__double2int_rd(fbB) << 2);
+                asm volatile("" : "+r"(kA), "+r"(kB));                  // one constant per ray: keep the sum out of the loop
                 float2 fi = make_float2((float)(s0 - ic), (float)(s0 - ic));
                 for (int i = s0; i <= s1; ++i) {
-                    tm_mbar_wait(&S.full[st], ph);
-                    // release the PREVIOUS stage here, where its loads have returned.  The reads went through the
-                    // generic proxy, the next copy into the stage comes through the async proxy: the fence orders
-                    // the two (without it the TMA engine was observed overwriting words that were still being read:
-                    // a few wrong rays per projection, not reproducible)
-                    if (prev >= 0) {
-                        tm_fence_proxy_async();
-                        __syncwarp();
-                        if (lane == 0) tm_mbar_arrive(&S.empty[prev]);
-                    }
-                    prev = st;
-                    const unsigned org = S.org[st];
+                    tl_wait_addr(bar, ph);
+                    // release the PREVIOUS stage here, where its loads have returned (the producer orders the
+                    // consumers' generic-proxy reads before its next async-proxy copy with a proxy fence)
+                    __syncwarp();
+                    if (lane == 0) tl_arrive_addr(prev + kTlEmptyOff);
+                    prev = bar;
+                    const unsigned org = __float_as_uint(al_lds(bar + kTlOrgOff));
                     const float2 ps = __ffma2_rn(fi, rs2, as2), pf = __ffma2_rn(fi, rf2, af2);
                     fi = __fadd2_rn(fi, kOne2);
                     const float2 xs = __fadd2_rd(ps, kMagic2), xf = __fadd2_rd(pf, kMagic2);     // bits = 0x4B400000 + floor
@@ -301,24 +354,20 @@ fp_tile_kernel(const __grid_constant__ TileParams P)
                     const float2 t0 = __ffma2_rn(wf, __ffma2_rn(v00, kNegOne2, v01), v00);       // row j
                     const float2 t1 = __ffma2_rn(wf, __ffma2_rn(v10, kNegOne2, v11), v10);       // row j + 1
                     acc = __fadd2_rn(acc, __ffma2_rn(ws, __ffma2_rn(t0, kNegOne2, t1), t0));
-                    if (++st == nst) {
-                        st = 0;
+                    bar += 8u;
+                    if (bar == bar_end) {
+                        bar = bar0;
                         ph ^= 1u;
                     }
                 }
             }
-            // a ray that misses the volume (or the degenerate ray) writes +0.0
-            const float oA = RA.i_last >= RA.i_first ? (float)(P.G.delta * RA.L) * acc.x : 0.0f;
-            const float oB = RB.i_last >= RB.i_first ? (float)(P.G.delta * RB.L) * acc.y : 0.0f;
-            if (liveA) P.out[((size_t)proj * P.nv + ivA) * P.nu + iuA] = oA;
-            if (liveB) P.out[((size_t)proj * P.nv + ivB) * P.nu + iuB] = oB;
-            if (liveA) n_samples += max(RA.i_last - RA.i_first + 1, 0);
-            if (liveB) n_samples += max(RB.i_last - RB.i_first + 1, 0);
+            if (liveA) P.out[outA] = scA * acc.x + 0.0f;
+            if (liveB) P.out[outB] = scB * acc.y + 0.0f;
         }
     }
     if (P.sample_count) block_count_samples(P.sample_count, n_samples);
 }
 
-constexpr size_t tile_smem_bytes() { return kTlTileBytes + sizeof(TlShared); }
+constexpr size_t tile_smem_bytes() { return kTlTileBytes + sizeof(TlShared) + kTlRayBytes; }
 
 }  // namespace fpk
