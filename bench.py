@@ -235,6 +235,9 @@ def run_backproject(args, torch, fp, cfg, geom, vol, proj, P, stream, world, ran
     vol_bytes, proj_bytes = vol.numel() * 4, cfg.nu * cfg.nv * 4
     algo = cfg.n_proj * (2 * vol_bytes + proj_bytes)        # read-modify-write of the volume once per projection
     achieved = algo / (ms * 1e-3) / 1e9
+    # poses of the aligned class take the transpose of the TMA-fed kernel unless the direct kernel is forced
+    aligned = P.plan(geom[0], cfg.nu, cfg.nv)[0] in (fp.KERNEL_ALIGNED, fp.KERNEL_TMA)
+    bp_kernel = "fp_bp_aligned_kernel" if aligned else "fp_backproject_kernel"
     line = {
         "metric": "512^3 cone-beam back-projections/s", "value": replicas_throughput(world, cfg.n_proj, ms * 1e-3),
         "unit": "projections/s", "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms,
@@ -243,7 +246,7 @@ def run_backproject(args, torch, fp, cfg, geom, vol, proj, P, stream, world, ran
         "clocks": clk, "gpu_launches": launches,
         "roofline": {"bound": "hbm", "achieved": achieved, "peak": peaks["hbm_gbs"], "unit": "GB/s",
                      "frac": achieved / peaks["hbm_gbs"], "traffic": None, "peak_kind": peak_kind,
-                     "kernel": "fp_backproject_kernel", "algorithmic_bytes_per_launch": algo},
+                     "kernel": bp_kernel, "algorithmic_bytes_per_launch": algo},
         "adjoint_check": {"lhs": lhs, "rhs": rhs, "rel_diff": abs(lhs - rhs) / abs(lhs)},
     }
     print(json.dumps(line))

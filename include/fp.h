@@ -171,7 +171,10 @@ fp_status fp_project_host(fp_ctx *ctx, const float *vol_host, int n_proj, const 
  * every sample of every ray receives voxel_size * ||r~|| * w * w * proj[ray] (same set-up, slices, taps and
  * weights; FP_OPT_INTERP applies).  fp32 reductions (RED.ADD.F32.FTZ: denormal contributions are flushed to
  * zero) in arbitrary order: results are reproducible only to
- * fp32 rounding of the sum.
+ * fp32 rounding of the sum.  Poses of the aligned class (the ones fp_plan gives FP_KERNEL_TMA / FP_KERNEL_ALIGNED)
+ * take fp_bp_aligned_kernel, the transpose of the TMA-fed forward kernel with the same fp32 positions and weights;
+ * all others -- and every pose with FP_OPT_KERNEL = FP_KERNEL_DIRECT -- the ray-driven scatter
+ * fp_backproject_kernel.  FP_OPT_FOV_CYLINDER is ignored (it would change the operator).
  *   proj_dev     device, fp32 [n_proj][nv][nu]
  *   vol_out_dev  device, fp32 [nx][ny][nz], fully overwritten (cleared first, also for n_proj = 0)
  */

@@ -15,7 +15,7 @@ CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libfp.so")
 SOURCES = [os.path.join(CSRC, "fp.cu")]
 HEADERS = [os.path.join(CSRC, "fp_kernels.cuh"), os.path.join(CSRC, "fp_setup.cuh"),
-           os.path.join(CSRC, "fp_aligned.cuh"), os.path.join(CSRC, "fp_tma.cuh"), os.path.join(CSRC, "fp_tex.cuh"), os.path.join(CSRC, "fp_probe.cuh"), os.path.join(CSRC, "fp_tile.cuh"),
+           os.path.join(CSRC, "fp_aligned.cuh"), os.path.join(CSRC, "fp_tma.cuh"), os.path.join(CSRC, "fp_tex.cuh"), os.path.join(CSRC, "fp_probe.cuh"), os.path.join(CSRC, "fp_tile.cuh"), os.path.join(CSRC, "fp_bp.cuh"),
            os.path.join(os.path.dirname(HERE), "include", "fp.h")]
 
 NVCC_FLAGS = [

@@ -17,6 +17,7 @@
 #include "fp_tma.cuh"
 #include "fp_tex.cuh"
 #include "fp_tile.cuh"
+#include "fp_bp.cuh"
 #include "fp_probe.cuh"
 
 using namespace fpk;
@@ -899,23 +900,64 @@ extern "C" fp_status fp_backproject(fp_ctx *c, const float *proj_dev, int n_proj
     if (n_proj == 0) return leave_stream(c, st);
     s = upload_geometry(c, n_proj, geom, nu, nv, false, st);
     if (s != FP_OK) return s;
-    BackprojectParams B;
-    B.G = c->G;
-    fill_layouts(c, vol_out_dev, false, B.lay);
-    B.proj = c->proj_dev;
-    B.in = proj_dev;
-    B.nu = nu;
-    B.nv = nv;
-    B.n_proj = n_proj;
-    const unsigned gl = (unsigned)((std::max(nu, nv) + kTileLane - 1) / kTileLane);
-    const unsigned gr = (unsigned)((std::max(nu, nv) + kTileRow - 1) / kTileRow);
-    dim3 grid(gl, gr, (unsigned)n_proj);
-    if (c->opt_interp == FP_INTERP_SPLINE)
-        fp_backproject_kernel<1><<<grid, kDirectThreads, 0, st>>>(B);
-    else
-        fp_backproject_kernel<0><<<grid, kDirectThreads, 0, st>>>(B);
-    FP_CUDA(c, cudaGetLastError());
-    c->last_launches += 1;
+    // plan: poses of the aligned class (fp_tma.cuh) take the transpose of the TMA-fed kernel, everything else --
+    // and everything with FP_KERNEL_DIRECT -- the ray-driven scatter.  The aligned kernel addresses the volume
+    // with 32-bit element indices.
+    std::vector<int> ids_al, ids_di;
+    const bool small = n_voxels(c) < 0xFFFFFFF0ull;
+    for (int p = 0; p < n_proj; ++p) {
+        const bool al = small && c->opt_kernel != FP_KERNEL_DIRECT && c->opt_kernel != FP_KERNEL_TEX &&
+                        c->opt_kernel != FP_KERNEL_HWLIN && plan_aligned(c, nullptr, geom + 12 * (size_t)p, nu, nv) > 0;
+        (al ? ids_al : ids_di).push_back(p);
+    }
+    s = ensure_ids(c, n_proj);
+    if (s != FP_OK) return s;
+    if (!ids_al.empty())
+        FP_CUDA(c, cudaMemcpyAsync(c->ids_dev, ids_al.data(), sizeof(int) * ids_al.size(), cudaMemcpyHostToDevice, st));
+    if (!ids_di.empty())
+        FP_CUDA(c, cudaMemcpyAsync(c->ids_dev + c->ids_cap, ids_di.data(), sizeof(int) * ids_di.size(), cudaMemcpyHostToDevice, st));
+    if (!ids_al.empty()) {
+        BpParams B;
+        memset(&B, 0, sizeof B);
+        B.T.G = c->G;
+        B.T.proj = c->proj_dev;
+        B.T.ids = c->ids_dev;
+        B.T.err_flag = reinterpret_cast<unsigned int *>(c->count_dev + 1);
+        B.T.nu = nu;
+        B.T.nv = nv;
+        B.T.n_sel = (int)ids_al.size();
+        B.T.group = std::max(1, std::min(c->opt_group, (int)ids_al.size()));
+        B.in = proj_dev;
+        B.vol = vol_out_dev;
+        dim3 grid((unsigned)((nu + kTmTU - 1) / kTmTU * B.T.group), (unsigned)((nv + kBpRows - 1) / kBpRows),
+                  (unsigned)((ids_al.size() + B.T.group - 1) / B.T.group));
+        if (c->opt_interp == FP_INTERP_SPLINE)
+            fp_bp_aligned_kernel<1><<<grid, kBpThreads, 0, st>>>(B);
+        else
+            fp_bp_aligned_kernel<0><<<grid, kBpThreads, 0, st>>>(B);
+        FP_CUDA(c, cudaGetLastError());
+        c->last_launches += 1;
+    }
+    if (!ids_di.empty()) {
+        BackprojectParams B;
+        B.G = c->G;
+        fill_layouts(c, vol_out_dev, false, B.lay);
+        B.proj = c->proj_dev;
+        B.ids = c->ids_dev + c->ids_cap;
+        B.in = proj_dev;
+        B.nu = nu;
+        B.nv = nv;
+        B.n_proj = (int)ids_di.size();
+        const unsigned gl = (unsigned)((std::max(nu, nv) + kTileLane - 1) / kTileLane);
+        const unsigned gr = (unsigned)((std::max(nu, nv) + kTileRow - 1) / kTileRow);
+        dim3 grid(gl, gr, (unsigned)ids_di.size());
+        if (c->opt_interp == FP_INTERP_SPLINE)
+            fp_backproject_kernel<1><<<grid, kDirectThreads, 0, st>>>(B);
+        else
+            fp_backproject_kernel<0><<<grid, kDirectThreads, 0, st>>>(B);
+        FP_CUDA(c, cudaGetLastError());
+        c->last_launches += 1;
+    }
     return leave_stream(c, st);
 }
 

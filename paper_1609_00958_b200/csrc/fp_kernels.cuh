@@ -200,7 +200,8 @@ struct BackprojectParams {
     GridDesc G;
     AxisLayout lay[3];                 // the OUTPUT volume [nx][ny][nz], indexed by the driving axis m
     const ProjDesc *proj;
-    const float *in;                   // [n_proj][nv][nu]
+    const int *ids;                    // [n_proj] projections this launch handles
+    const float *in;                   // [all projections of the call][nv][nu]
     int nu, nv, n_proj;
 };
 
@@ -208,7 +209,7 @@ template <int INTERP>
 __global__ void __launch_bounds__(kDirectThreads)
 fp_backproject_kernel(const __grid_constant__ BackprojectParams P)
 {
-    const int proj = blockIdx.z;
+    const int proj = P.ids[blockIdx.z];
     const ProjDesc *pd = P.proj + proj;
     const int lane = threadIdx.x & 31, row = threadIdx.x >> 5;
     const bool lane_v = pd->lane_v != 0;

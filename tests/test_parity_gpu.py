@@ -517,6 +517,32 @@ def test_backprojection_c1_parity_and_adjoint_identity_at_c3_size(torch, fp, syn
     assert abs(lhs - rhs) <= 2e-5 * abs(lhs), (lhs, rhs)
 
 
+@pytest.mark.parametrize("interp", [0, 1])
+def test_backprojection_aligned_kernel_and_ray_driven_kernel_against_the_oracle(torch, fp, synth, oracle, interp):
+    """Circular-orbit poses take fp_bp_aligned_kernel (the transpose of the TMA-fed kernel), FP_KERNEL_DIRECT forces
+    the ray-driven scatter: both against the oracle on C2 (192 detector rows = a ragged row block, 11 poses = a
+    short last group, both driving axes and blocks where the axis switches)."""
+    cfg = synth.CONFIGS["C2"]
+    geom = synth.make_geometry(cfg)[np.r_[0:180:17]]
+    rng = np.random.default_rng(77 + interp)
+    y = rng.uniform(-1.0, 2.0, size=(len(geom), cfg.nv, cfg.nu)).astype(np.float32)
+    yd = torch.from_numpy(y).cuda()
+    with fp.Projector(*cfg.n, cfg.voxel_size, cfg.origin) as P:
+        P.set_option(fp.OPT_INTERP, interp)
+        assert all(P.plan(g, cfg.nu, cfg.nv)[0] in (fp.KERNEL_TMA, fp.KERNEL_ALIGNED) for g in geom)
+        g2 = P.backproject(yd, geom, cfg.nu, cfg.nv).cpu().numpy().astype(np.float64)
+        assert P.last_launch_count() == 1
+        P.check()
+        P.set_option(fp.OPT_KERNEL, fp.KERNEL_DIRECT)
+        g1 = P.backproject(yd, geom, cfg.nu, cfg.nv).cpu().numpy().astype(np.float64)
+    ref = oracle.backproject(y.astype(np.float64), cfg.n, cfg.voxel_size, cfg.origin, geom, kernel=interp, threads=oracle.host_cores())
+    tol = bp_tolerance(oracle, y.astype(np.float64), cfg.n, cfg.voxel_size, cfg.origin, geom, interp)
+    for name, g in (("aligned", g2), ("ray-driven", g1)):
+        err = np.abs(g - ref)
+        assert np.all(err <= tol), (name, float(np.max(err / np.maximum(tol, 1e-300))))
+    assert np.abs(ref).max() > 1.0
+
+
 def test_backprojection_c3_size_sampled_voxels(torch, fp, synth, oracle):
     """Element by element at full size: fp_backproject on the 512^3 grid of C3 (four poses, both driving axes),
     compared on 2^18 seeded voxels plus the volume's corners and centre,
