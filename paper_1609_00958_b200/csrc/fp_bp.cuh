@@ -36,9 +36,25 @@ struct __align__(16) BpShared {
     TmShared S;
     // per (stage, column): element index of (row j, window centre) and of (row j + 1, window centre) in the volume
     // (0xFFFFFFFF: that row is outside the volume or the column has no sample on the slice), weight bits of u
+    // .w = 1: neighbouring detector rows are more than half a voxel apart in z on this slice, so at most two
+    // neighbouring lanes share a word and the warp merges them before the reduction (see the kernel)
     uint4 tap[kTmSB][kTmTU];
     int zbase[2];                      // per batch parity: z of the window centre
+    double drho;                       // |r_z(row + 1) - r_z(row)|, grid units
 };
+
+// Predicated fp32 reduction in L2 (no branch around it).
+__device__ __forceinline__ void bp_red(float *p, float v, bool on)
+{
+    asm volatile(
+        "{\n"
+        ".reg .pred q;\n"
+        "setp.ne.b32 q, %2, 0;\n"
+        "@q red.global.add.f32 [%0], %1;\n"
+        "}\n" ::"l"(p),
+        "f"(v), "r"((int)on)
+        : "memory");
+}
 
 // Planning warp, one batch: lane = (slice s of the batch) * 8 + column c.  The same fp64 plan as tm_produce_batch
 // (fp_tma.cuh) -- volume row j = floor(p_slow) and weight u per (slice, column), centre of the batch's z window --
@@ -71,7 +87,8 @@ __device__ __forceinline__ void bp_plan_batch(BpShared &B, const BpParams &P, in
     const bool r0 = live && winok && j >= 0 && j < S.n_s, r1 = live && winok && j + 1 >= 0 && j + 1 < S.n_s;
     const long long e0 = pass == 0 ? ((long long)i * ny + j) * nz : ((long long)j * ny + i) * nz;
     const long long estep = pass == 0 ? nz : ny * nz;
-    const uint4 tap = make_uint4(r0 ? (unsigned)e0 : 0xFFFFFFFFu, r1 ? (unsigned)(e0 + estep) : 0xFFFFFFFFu, __float_as_uint(u), 0u);
+    const unsigned merge = fabs(t) * B.drho > 0.505 ? 1u : 0u;
+    const uint4 tap = make_uint4(r0 ? (unsigned)e0 : 0xFFFFFFFFu, r1 ? (unsigned)(e0 + estep) : 0xFFFFFFFFu, __float_as_uint(u), merge);
 #pragma unroll
     for (int ss = 0; ss < kTmSB; ++ss) {
         if (gb > 0) tm_mbar_wait(&S.empty[ss], (gb - 1) & 1);
@@ -125,6 +142,7 @@ fp_bp_aligned_kernel(const __grid_constant__ BpParams P)
             S.s[2] = s[2];
             S.rho_first = al_rho(g, T.G, row0, s[2]);
             S.rho_last = al_rho(g, T.G, min(row0 + kBpRows, T.nv) - 1, s[2]);
+            B.drho = fabs(g[11]) / T.G.delta;
 #pragma unroll
             for (int k = 0; k < kTmSB; ++k) {
                 tm_mbar_init(&S.full[k], 1);
@@ -192,7 +210,8 @@ fp_bp_aligned_kernel(const __grid_constant__ BpParams P)
                     const double t0 = S.t0[par][c];
                     a[c] = make_float2((float)fma(t0, rho0, off), (float)fma(t0, rho1, off));
                 }
-#pragma unroll
+                // not unrolled: the body (8 columns x 16 reductions) already fills the instruction cache
+#pragma unroll 1
                 for (int s = 0; s < kTmSB; ++s) {
                     if (s) tm_mbar_wait(&S.full[s], par);
                     const float2 fs = make_float2((float)s, (float)s);
@@ -209,24 +228,41 @@ fp_bp_aligned_kernel(const __grid_constant__ BpParams P)
                         const float2 hi = __fmul2_rn(yb[c], make_float2(uy, uy));
                         const float2 lo = __ffma2_rn(hi, kNegOne2, yb[c]);
                         const float2 t01 = __fmul2_rn(lo, wz), t11 = __fmul2_rn(hi, wz);
-                        const float2 t00 = __ffma2_rn(t01, kNegOne2, lo), t10 = __ffma2_rn(t11, kNegOne2, hi);
-                        const int k0 = (int)__float_as_uint(x.x) + zb0, k1 = (int)__float_as_uint(x.y) + zb1;   // z of the lower tap
+                        float2 t00 = __ffma2_rn(t01, kNegOne2, lo), t10 = __ffma2_rn(t11, kNegOne2, hi);
+                        float2 t01m = t01, t11m = t11;
+                        int k0 = (int)__float_as_uint(x.x) + zb0, k1 = (int)__float_as_uint(x.y) + zb1;   // z of the lower tap
+                        if (tp.w) {
+                            // lanes are neighbouring detector rows, z is monotone in the row, rows are more than half a
+                            // voxel apart: a word is shared by at most two neighbouring lanes.  The first of them adds
+                            // the second one's values to its own and the second one drops out: every reduction
+                            // instruction then carries each word once (half the L2 reduction operations).
+                            const unsigned full = 0xffffffffu;
+                            const int k0n = __shfl_down_sync(full, k0, 1), k0p = __shfl_up_sync(full, k0, 1);
+                            const int k1n = __shfl_down_sync(full, k1, 1), k1p = __shfl_up_sync(full, k1, 1);
+                            const bool take0 = lane < 31 && k0n == k0, take1 = lane < 31 && k1n == k1;
+                            const float a00 = __shfl_down_sync(full, t00.x, 1), a01 = __shfl_down_sync(full, t01m.x, 1);
+                            const float a10 = __shfl_down_sync(full, t10.x, 1), a11 = __shfl_down_sync(full, t11m.x, 1);
+                            const float b00 = __shfl_down_sync(full, t00.y, 1), b01 = __shfl_down_sync(full, t01m.y, 1);
+                            const float b10 = __shfl_down_sync(full, t10.y, 1), b11 = __shfl_down_sync(full, t11m.y, 1);
+                            if (take0) { t00.x += a00; t01m.x += a01; t10.x += a10; t11m.x += a11; }
+                            if (take1) { t00.y += b00; t01m.y += b01; t10.y += b10; t11m.y += b11; }
+                            if (lane > 0 && k0p == k0) k0 = 0x40000000;
+                            if (lane > 0 && k1p == k1) k1 = 0x40000000;
+                        }
                         const bool a0 = (unsigned)k0 < nz, a1 = (unsigned)(k0 + 1) < nz;
                         const bool b0 = (unsigned)k1 < nz, b1 = (unsigned)(k1 + 1) < nz;
-                        if (tp.x != 0xFFFFFFFFu) {
-                            float *q0 = vol + ((long long)tp.x + k0), *q1 = vol + ((long long)tp.x + k1);
-                            if (a0) atomicAdd(q0, t00.x);
-                            if (a1) atomicAdd(q0 + 1, t01.x);
-                            if (b0) atomicAdd(q1, t00.y);
-                            if (b1) atomicAdd(q1 + 1, t01.y);
-                        }
-                        if (tp.y != 0xFFFFFFFFu) {
-                            float *q0 = vol + ((long long)tp.y + k0), *q1 = vol + ((long long)tp.y + k1);
-                            if (a0) atomicAdd(q0, t10.x);
-                            if (a1) atomicAdd(q0 + 1, t11.x);
-                            if (b0) atomicAdd(q1, t10.y);
-                            if (b1) atomicAdd(q1 + 1, t11.y);
-                        }
+                        const bool r0 = tp.x != 0xFFFFFFFFu, r1 = tp.y != 0xFFFFFFFFu;
+                        float *qa = vol + ((long long)tp.x + k0), *qb = vol + ((long long)tp.x + k1);
+                        bp_red(qa, t00.x, r0 && a0);
+                        bp_red(qa + 1, t01m.x, r0 && a1);
+                        bp_red(qb, t00.y, r0 && b0);
+                        bp_red(qb + 1, t01m.y, r0 && b1);
+                        qa = vol + ((long long)tp.y + k0);
+                        qb = vol + ((long long)tp.y + k1);
+                        bp_red(qa, t10.x, r1 && a0);
+                        bp_red(qa + 1, t11m.x, r1 && a1);
+                        bp_red(qb, t10.y, r1 && b0);
+                        bp_red(qb + 1, t11m.y, r1 && b1);
                     }
                     // the plan of this stage has been read
                     __syncwarp();
