@@ -60,16 +60,22 @@ struct TlCorner {                      // one corner ray, parametrised along the
     double s_m, s_a, s_b, rt_a, rt_b;
 };
 
+struct TlPass {                        // one pass = the tile's rays whose driving axis is m
+    int lo, hi;                        // union of their slice ranges; hi < lo: no such ray
+    int size_r, size_c, staged;        // box classes; staged = 1: staged pass, 0: those rays take the direct path
+    int pad_;
+};
+
 struct __align__(16) TlShared {
     // the consumers walk these three arrays with ONE running byte address (stage * 8): keep them 8 bytes per stage
     // and in this order (kTlEmptyOff, kTlOrgOff below)
     unsigned long long full[kTlStagesMax], empty[kTlStagesMax];
     uint2 org[kTlStagesMax];           // .x per stage: byte address of tile word (0, 0) minus (js0 * pitch + kf0) * 4 terms, see below
     unsigned long long sink;           // barrier nobody waits on: takes the release of "the stage before the first"
-    TlCorner corner[4];
-    int m[4];                          // driving axis (+ 4 if r_m < 0) of the corner rays; -1: degenerate
-    int lo, hi;                        // slice range of the block (union of its rays' ranges)
-    int size_r, size_c, staged;        // box classes; staged = 1: staged path, 0: direct path
+    TlCorner corner[3][4];             // per pass (= driving axis m): the four corner rays parametrised along m
+    double cr[4][3];                   // the corner rays' directions r (Eq. 1), grid units
+    double cs[3];                      // the source, grid units
+    TlPass pass[3];
 };
 
 constexpr unsigned kTlEmptyOff = 8u * kTlStagesMax, kTlOrgOff = 16u * kTlStagesMax, kTlSinkOff = 24u * kTlStagesMax;
@@ -77,7 +83,9 @@ static_assert(offsetof(TlShared, empty) == kTlEmptyOff && offsetof(TlShared, org
               "TlShared layout");
 // fp64 parameters of the two rays of every consumer thread, parked in shared memory while the sampling loop runs (they
 // are needed once per segment only; in registers they would cost a third of the occupancy): [4][kTlConsumers] double2
-constexpr unsigned kTlRayBytes = 4u * kTlConsumers * 16u;
+// plus one slot per pass holding a corner ray's parameters: what a ray reads in a pass that is not its own
+constexpr int kTlRaySlots = kTlConsumers + 4;
+constexpr unsigned kTlRayBytes = 4u * kTlRaySlots * 16u;
 
 __device__ __forceinline__ void tl_wait_addr(unsigned bar, unsigned parity)
 {
@@ -119,6 +127,20 @@ __device__ __forceinline__ float tl_direct_ray(const RaySetup &R, const AxisLayo
     return acc;
 }
 
+// Direct path for one pixel, set-up included (kept out of line: only tiles whose box does not fit a stage, or whose
+// z-driven rays have no y-fastest copy to be staged from, come here).
+template <int INTERP>
+__device__ __noinline__ float tl_direct_pixel(const double *g, const GridDesc &G, const AxisLayout *lay, int iu, int iv)
+{
+    const RaySetup R = ray_setup(g, G, iu, iv);
+    return (float)(G.delta * R.L) * tl_direct_ray<INTERP>(R, lay);
+}
+
+__device__ __forceinline__ void tl_mbar_inval(unsigned long long *bar)
+{
+    asm volatile("mbarrier.inval.shared::cta.b64 [%0];" ::"r"(tm_smem(bar)) : "memory");
+}
+
 template <int INTERP>
 __global__ void __launch_bounds__(kTlThreads, 3)
 fp_tile_kernel(const __grid_constant__ TileParams P)
@@ -135,21 +157,26 @@ fp_tile_kernel(const __grid_constant__ TileParams P)
     const double *g = pd->g;
     const int tu0 = blockIdx.x * kTlU, tv0 = blockIdx.y * kTlV;
 
-    // ---- corner rays (Eqs. 1-5): the tile's rectangle, also where it sticks out past the detector edge
+    // ---- corner rays (Eq. 1, the operations of ray_setup): the tile's rectangle, also where it sticks out past the
+    //      detector edge
     if (tid < 4) {
         const int iu = tu0 + ((tid & 1) ? kTlU - 1 : 0), iv = tv0 + ((tid & 2) ? kTlV - 1 : 0);
-        const RaySetup R = ray_setup(g, P.G, iu, iv);
-        TlCorner C;
-        C.s_m = R.s_m; C.s_a = R.s_a; C.s_b = R.s_b; C.rt_a = R.rt_a; C.rt_b = R.rt_b;
-        S.corner[tid] = C;
-        // driving axis AND sense of the corner ray: code m for r_m > 0, m + 4 for r_m < 0 (the rays between four
-        // corners lie in one convex cone { r : r_m >= |r_a| } only if the sense agrees as well)
-        const double rm = ((g[3 + R.m] + (double)iu * g[6 + R.m]) + (double)iv * g[9 + R.m]) - g[R.m];
-        S.m[tid] = R.L > 0.0 ? R.m + (rm < 0.0 ? 4 : 0) : -1;
+#pragma unroll
+        for (int a = 0; a < 3; ++a) {
+            const double D = __dadd_rn(__dadd_rn(g[3 + a], __dmul_rn((double)iu, g[6 + a])), __dmul_rn((double)iv, g[9 + a]));
+            const double s = __ddiv_rn(__dsub_rn(g[a], P.G.origin[a]), P.G.delta);
+            const double d = __ddiv_rn(__dsub_rn(D, P.G.origin[a]), P.G.delta);
+            S.cr[tid][a] = __dsub_rn(d, s);
+            if (tid == 0) S.cs[a] = s;
+        }
     }
     if (tid == 0) {
-        S.lo = 0x7fffffff;
-        S.hi = -1;
+#pragma unroll
+        for (int m = 0; m < 3; ++m) {
+            S.pass[m].lo = 0x7fffffff;
+            S.pass[m].hi = -1;
+            S.pass[m].staged = 0;
+        }
 #pragma unroll
         for (int k = 0; k < kTlStagesMax; ++k) {
             tm_mbar_init(&S.full[k], 1);
@@ -161,14 +188,16 @@ fp_tile_kernel(const __grid_constant__ TileParams P)
     __syncthreads();
 
     // ---- per-ray exact set-up (fp64, Eqs. 1-6 and the exact slice range); lanes run along the detector axis that
-    //      maps onto the contiguous in-plane axis of the tile's driving axis (neighbouring lanes -> neighbouring words)
-    const int m_code = S.m[0], m_tile = m_code & 3;
-    const bool same_m = m_code >= 0 && S.m[1] == m_code && S.m[2] == m_code && S.m[3] == m_code && (m_tile != 2 || P.z_staged);
-    const int fa = m_tile == 2 ? 1 : 2;                       // fast in-plane axis: z, or y on the permuted copy
-    const bool lanes_v = same_m && fabs(g[9 + fa]) > fabs(g[6 + fa]);
+    //      maps onto the contiguous in-plane axis of the first corner's driving axis (neighbouring lanes ->
+    //      neighbouring words)
+    bool lanes_v;
+    {
+        const double r0 = fabs(S.cr[0][0]), r1 = fabs(S.cr[0][1]), r2 = fabs(S.cr[0][2]);
+        const int m0 = (r2 > r1 && r2 > r0) ? 2 : (r1 > r0 ? 1 : 0);
+        const int fa = m0 == 2 ? 1 : 2;                       // fast in-plane axis: z, or y on the permuted copy
+        lanes_v = fabs(g[9 + fa]) > fabs(g[6 + fa]);
+    }
     int iuA = 0, ivA = 0, iuB = 0, ivB = 0;
-    RaySetup RA, RB;
-    bool liveA = false, liveB = false;
     if (!producer) {
         const int w = tid >> 5;
         if (!lanes_v) {                                       // 32 lanes along u; rows w and w + 8
@@ -180,34 +209,71 @@ fp_tile_kernel(const __grid_constant__ TileParams P)
             iuA = tu0 + 2 * (2 * w + (lane >> 4));
             iuB = iuA + 1;
         }
-        liveA = iuA < P.nu && ivA < P.nv;
-        liveB = iuB < P.nu && ivB < P.nv;
-        RA = ray_setup(g, P.G, min(iuA, P.nu - 1), min(ivA, P.nv - 1));
-        RB = ray_setup(g, P.G, min(iuB, P.nu - 1), min(ivB, P.nv - 1));
-        if (same_m) {
+    }
+    const bool liveA = !producer && iuA < P.nu && ivA < P.nv, liveB = !producer && iuB < P.nu && ivB < P.nv;
+    // a thread's state across the passes: driving axis of its two rays (3: the ray misses the volume), the scales
+    // Delta ||r~||; the fp64 parameters go to shared memory (read back once per segment)
+    int mA = 3, mB = 3, n_samples = 0;
+    float scA = 0.0f, scB = 0.0f;
+    double2 *rayp = reinterpret_cast<double2 *>(tl_smem_raw + kTlTileBytes + sizeof(TlShared));
+    if (!producer) {
+        const RaySetup RA = ray_setup(g, P.G, min(iuA, P.nu - 1), min(ivA, P.nv - 1));
+        const RaySetup RB = ray_setup(g, P.G, min(iuB, P.nu - 1), min(ivB, P.nv - 1));
+        if (RA.i_last >= RA.i_first) { mA = RA.m; scA = (float)(P.G.delta * RA.L); }
+        if (RB.i_last >= RB.i_first) { mB = RB.m; scB = (float)(P.G.delta * RB.L); }
+        rayp[0 * kTlRaySlots + tid] = make_double2(RA.s_a, RA.rt_a);
+        rayp[1 * kTlRaySlots + tid] = make_double2(RA.s_b, RA.rt_b);
+        rayp[2 * kTlRaySlots + tid] = make_double2(RB.s_a, RB.rt_a);
+        rayp[3 * kTlRaySlots + tid] = make_double2(RB.s_b, RB.rt_b);
+        if (liveA) n_samples += max(RA.i_last - RA.i_first + 1, 0);
+        if (liveB) n_samples += max(RB.i_last - RB.i_first + 1, 0);
+        // slice range of every pass: the union over its rays
+#pragma unroll
+        for (int m = 0; m < 3; ++m) {
             int lo = 0x7fffffff, hi = -1;
-            if (RA.i_last >= RA.i_first) { lo = RA.i_first; hi = RA.i_last; }
-            if (RB.i_last >= RB.i_first) { lo = min(lo, RB.i_first); hi = max(hi, RB.i_last); }
+            if (mA == m) { lo = RA.i_first; hi = RA.i_last; }
+            if (mB == m) { lo = min(lo, RB.i_first); hi = max(hi, RB.i_last); }
             lo = __reduce_min_sync(0xffffffffu, lo);
             hi = __reduce_max_sync(0xffffffffu, hi);
             if (lane == 0 && hi >= lo) {
-                atomicMin(&S.lo, lo);
-                atomicMax(&S.hi, hi);
+                atomicMin(&S.pass[m].lo, lo);
+                atomicMax(&S.pass[m].hi, hi);
             }
         }
+        // a ray that misses the volume (or the degenerate ray) writes +0.0
+        if (liveA && mA == 3) P.out[((size_t)proj * P.nv + ivA) * P.nu + iuA] = 0.0f;
+        if (liveB && mB == 3) P.out[((size_t)proj * P.nv + ivB) * P.nu + iuB] = 0.0f;
     }
     __syncthreads();
-    // ---- does the tile qualify for the staged path?  Box of the corner quadrilateral at both ends of the slice range
-    //      (every corner point is affine in the slice index, so the extents are largest at one of the ends)
-    if (tid == 0) {
+    // ---- plan of the passes (thread m plans pass m).  In pass m EVERY ray of the tile is parametrised along axis m
+    //      (r~ = r / r_m, Eq. 4): if r_m has one sign at the four corners it has that sign on the whole tile (r is
+    //      affine in the pixel), the map pixel -> intersection point with slice i is projective, and all rays cut the
+    //      slice inside the quadrilateral of the corner rays' points.  The pass copies the bounding box of that
+    //      quadrilateral; the rays whose driving axis IS m (Eq. 2) sample it, the others go through the motions with
+    //      the first corner's parameters and drop the result.  Box classes from both ends of the slice range (every
+    //      corner point is affine in the slice index, so the extents are largest at one of the ends).
+    if (tid < 3 && S.pass[tid].hi >= S.pass[tid].lo) {
+        const int m = tid, ta = axis_slow(m), tb = axis_fast(m);
+        TlPass &Q = S.pass[m];
+        const double r0 = S.cr[0][m], r1 = S.cr[1][m], r2 = S.cr[2][m], r3 = S.cr[3][m];
+        const bool one_sign = (r0 > 0.0 && r1 > 0.0 && r2 > 0.0 && r3 > 0.0) || (r0 < 0.0 && r1 < 0.0 && r2 < 0.0 && r3 < 0.0);
         int size_r = -1, size_c = -1;
-        if (same_m && S.hi >= S.lo) {
+        if (one_sign && (m != 2 || P.z_staged)) {
+            for (int c = 0; c < 4; ++c) {
+                TlCorner C;
+                C.s_m = S.cs[m];
+                C.s_a = S.cs[ta];
+                C.s_b = S.cs[tb];
+                C.rt_a = __ddiv_rn(S.cr[c][ta], S.cr[c][m]);
+                C.rt_b = __ddiv_rn(S.cr[c][tb], S.cr[c][m]);
+                S.corner[m][c] = C;
+            }
             int rows = 0, cols = 0;
             for (int e = 0; e < 2; ++e) {
-                const int i = e ? S.hi : S.lo;
+                const int i = e ? Q.hi : Q.lo;
                 double smin = 1e300, smax = -1e300, fmin_ = 1e300, fmax_ = -1e300;
                 for (int c = 0; c < 4; ++c) {
-                    const TlCorner &C = S.corner[c];
+                    const TlCorner &C = S.corner[m][c];
                     const double ps = p_of_i(C.s_a, C.s_m, C.rt_a, i), pf = p_of_i(C.s_b, C.s_m, C.rt_b, i);
                     smin = fmin(smin, ps); smax = fmax(smax, ps);
                     fmin_ = fmin(fmin_, pf); fmax_ = fmax(fmax_, pf);
@@ -221,35 +287,54 @@ fp_tile_kernel(const __grid_constant__ TileParams P)
                 if (rows <= tl_rows(k)) size_r = k;
                 if (cols <= tl_cols(k)) size_c = k;
             }
+            // the slot a ray reads in a pass that is not its own: the first corner's parameters
+            const TlCorner &C0 = S.corner[m][0];
+#pragma unroll
+            for (int q = 0; q < 4; ++q)
+                rayp[q * kTlRaySlots + kTlConsumers + m] = (q & 1) ? make_double2(C0.s_b, C0.rt_b) : make_double2(C0.s_a, C0.rt_a);
         }
-        S.size_r = max(size_r, 0);
-        S.size_c = max(size_c, 0);
-        S.staged = size_r >= 0 && size_c >= 0;
+        Q.size_r = max(size_r, 0);
+        Q.size_c = max(size_c, 0);
+        Q.staged = size_r >= 0 && size_c >= 0;
     }
     __syncthreads();
 
-    int n_samples = 0;
-    if (!S.staged) {
-        // ---- direct path (mixed driving axes, oversized box, or nothing to sample)
-        if (!producer) {
-            const float a = tl_direct_ray<INTERP>(RA, P.lay), b = tl_direct_ray<INTERP>(RB, P.lay);
-            if (liveA) P.out[((size_t)proj * P.nv + ivA) * P.nu + iuA] = (float)(P.G.delta * RA.L) * a;
-            if (liveB) P.out[((size_t)proj * P.nv + ivB) * P.nu + iuB] = (float)(P.G.delta * RB.L) * b;
-            if (liveA) n_samples += max(RA.i_last - RA.i_first + 1, 0);
-            if (liveB) n_samples += max(RB.i_last - RB.i_first + 1, 0);
+    bool ring_used = false;
+    for (int m = 0; m < 3; ++m) {
+        const int lo = S.pass[m].lo, hi = S.pass[m].hi;
+        if (hi < lo) continue;                                           // no ray of the tile has this driving axis
+        if (!S.pass[m].staged) {
+            // ---- direct path for the rays of this axis (oversized box, no staged copy for z, r_m changing sign)
+            if (liveA && mA == m) P.out[((size_t)proj * P.nv + ivA) * P.nu + iuA] = tl_direct_pixel<INTERP>(g, P.G, P.lay, iuA, ivA);
+            if (liveB && mB == m) P.out[((size_t)proj * P.nv + ivB) * P.nu + iuB] = tl_direct_pixel<INTERP>(g, P.G, P.lay, iuB, ivB);
+            continue;
         }
-    } else {
-        const int lo = S.lo, hi = S.hi;
+        if (ring_used) {
+            // a second staged pass (about 4 % of C4's tiles): the ring starts over with its own stage size
+            __syncthreads();
+            if (tid == 0) {
+                for (int k = 0; k < kTlStagesMax; ++k) {
+                    tl_mbar_inval(&S.full[k]);
+                    tl_mbar_inval(&S.empty[k]);
+                    tm_mbar_init(&S.full[k], 1);
+                    tm_mbar_init(&S.empty[k], kTlConsumers / 32);
+                }
+                asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+            }
+            __syncthreads();
+        }
+        ring_used = true;
         const int n_slices = hi - lo + 1;
-        const int rows = tl_rows(S.size_r), cols = tl_cols(S.size_c);
+        const int size_r = S.pass[m].size_r, size_c = S.pass[m].size_c;
+        const int rows = tl_rows(size_r), cols = tl_cols(size_c);
         const unsigned pitchB = (unsigned)cols * 4u, boxB = (unsigned)(rows * cols * 4), stageB = tl_stage_stride(rows, cols);
         const int nst = min(kTlStagesMax, (int)(kTlTileBytes / stageB));   // stages in flight
         if (producer) {
             // lane = slice-in-batch * 8 + corner * 2 + coordinate; batches of four slices
             const int sb = lane >> 3, cc = (lane >> 1) & 3, co = lane & 1;
-            const TlCorner C = S.corner[cc];
+            const TlCorner C = S.corner[m][cc];
             const double s_t = co ? C.s_b : C.s_a, rt_t = co ? C.rt_b : C.rt_a;
-            const CUtensorMap *map = &P.map[m_tile][S.size_r][S.size_c];
+            const CUtensorMap *map = &P.map[m][size_r][size_c];
             int st = 0;
             unsigned ph = 0;                                             // parity of the empty phase to wait for (from the second round on)
             for (int n0 = 0; n0 < n_slices; n0 += 4) {
@@ -277,7 +362,7 @@ fp_tile_kernel(const __grid_constant__ TileParams P)
                         const int ii = lo + n;
                         // tensor dimensions, fastest first: m = x: (z, y, x); m = y: (z, y, x) with the slow axis x;
                         // m = z: the y-fastest copy (y, x, z)
-                        if (m_tile == 1)
+                        if (m == 1)
                             tm_load_3d(map, dst, &S.full[st], kf0, ii, js0);
                         else
                             tm_load_3d(map, dst, &S.full[st], kf0, js0, ii);
@@ -292,20 +377,9 @@ fp_tile_kernel(const __grid_constant__ TileParams P)
         } else {
             const float2 kMagic2 = make_float2(12582912.0f, 12582912.0f), kNegMagic2 = make_float2(-12582912.0f, -12582912.0f);
             const float2 kNegOne2 = make_float2(-1.0f, -1.0f), kOne2 = make_float2(1.0f, 1.0f);
-            // what the loop needs of the two rays: the fp64 parameters go to shared memory (read back once per
-            // segment), the rest is folded into two scales and a count -- RA / RB are dead from here on
-            double2 *rayp = reinterpret_cast<double2 *>(tl_smem_raw + kTlTileBytes + sizeof(TlShared)) + tid;
-            rayp[0 * kTlConsumers] = make_double2(RA.s_a, RA.rt_a);
-            rayp[1 * kTlConsumers] = make_double2(RA.s_b, RA.rt_b);
-            rayp[2 * kTlConsumers] = make_double2(RB.s_a, RB.rt_a);
-            rayp[3 * kTlConsumers] = make_double2(RB.s_b, RB.rt_b);
-            const double s_m = S.corner[0].s_m;                          // the source's coordinate along m: the same for every ray
-            // scale Delta ||r~||; a ray that misses the volume (or the degenerate ray) writes +0.0
-            const float scA = RA.i_last >= RA.i_first ? (float)(P.G.delta * RA.L) : 0.0f;
-            const float scB = RB.i_last >= RB.i_first ? (float)(P.G.delta * RB.L) : 0.0f;
-            if (liveA) n_samples += max(RA.i_last - RA.i_first + 1, 0);
-            if (liveB) n_samples += max(RB.i_last - RB.i_first + 1, 0);
-            const size_t outA = ((size_t)proj * P.nv + ivA) * P.nu + iuA, outB = ((size_t)proj * P.nv + ivB) * P.nu + iuB;
+            const double s_m = S.cs[m];                                  // the source's coordinate along m: the same for every ray
+            // a ray of another driving axis reads the pass's corner slot instead of its own
+            const double2 *rpA = rayp + (mA == m ? tid : kTlConsumers + m), *rpB = rayp + (mB == m ? tid : kTlConsumers + m);
 
             float2 acc = make_float2(0.0f, 0.0f);
             // one running address walks full[], empty[] (+ kTlEmptyOff) and org[] (+ kTlOrgOff)
@@ -315,8 +389,8 @@ fp_tile_kernel(const __grid_constant__ TileParams P)
             for (int s0 = lo; s0 <= hi; s0 += kSegment) {
                 const int s1 = min(s0 + kSegment - 1, hi), ic = (s0 + s1) >> 1;
                 // fp64 anchors at the segment's middle slice, split into integer voxel index + fraction
-                const double2 qa = rayp[0 * kTlConsumers], qb = rayp[1 * kTlConsumers];
-                const double2 qc = rayp[2 * kTlConsumers], qd = rayp[3 * kTlConsumers];
+                const double2 qa = rpA[0 * kTlRaySlots], qb = rpA[1 * kTlRaySlots];
+                const double2 qc = rpB[2 * kTlRaySlots], qd = rpB[3 * kTlRaySlots];
                 const double paA = p_of_i(qa.x, s_m, qa.y, ic), pbA = p_of_i(qb.x, s_m, qb.y, ic);
                 const double paB = p_of_i(qc.x, s_m, qc.y, ic), pbB = p_of_i(qd.x, s_m, qd.y, ic);
                 // increments along the two in-plane axes of both rays (packed: .x = ray A, .y = ray B)
@@ -361,8 +435,8 @@ fp_tile_kernel(const __grid_constant__ TileParams P)
                     }
                 }
             }
-            if (liveA) P.out[outA] = scA * acc.x + 0.0f;
-            if (liveB) P.out[outB] = scB * acc.y + 0.0f;
+            if (liveA && mA == m) P.out[((size_t)proj * P.nv + ivA) * P.nu + iuA] = scA * acc.x + 0.0f;
+            if (liveB && mB == m) P.out[((size_t)proj * P.nv + ivB) * P.nu + iuB] = scB * acc.y + 0.0f;
         }
     }
     if (P.sample_count) block_count_samples(P.sample_count, n_samples);
