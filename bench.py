@@ -238,6 +238,7 @@ def run_backproject(args, torch, fp, cfg, geom, vol, proj, P, stream, world, ran
     # poses of the aligned class take the transpose of the TMA-fed kernel unless the direct kernel is forced
     aligned = P.plan(geom[0], cfg.nu, cfg.nv)[0] in (fp.KERNEL_ALIGNED, fp.KERNEL_TMA)
     bp_kernel = "fp_bp_aligned_kernel" if aligned else "fp_backproject_kernel"
+    cap, stale = captured_traffic(cfg.name, bp_kernel, args.interp)
     line = {
         "metric": "512^3 cone-beam back-projections/s", "value": replicas_throughput(world, cfg.n_proj, ms * 1e-3),
         "unit": "projections/s", "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms,
@@ -245,7 +246,10 @@ def run_backproject(args, torch, fp, cfg, geom, vol, proj, P, stream, world, ran
         "config": {"workload": workload_name(cfg), "op": "backproject", "interpolation": args.interp},
         "clocks": clk, "gpu_launches": launches,
         "roofline": {"bound": "hbm", "achieved": achieved, "peak": peaks["hbm_gbs"], "unit": "GB/s",
-                     "frac": achieved / peaks["hbm_gbs"], "traffic": None, "peak_kind": peak_kind,
+                     "frac": achieved / peaks["hbm_gbs"],
+                     "traffic": cap["dram_bytes"] if (cap is not None and not stale) else None,
+                     "traffic_source": (cap["source"] if (cap is not None and not stale) else None),
+                     "peak_kind": peak_kind,
                      "kernel": bp_kernel, "algorithmic_bytes_per_launch": algo},
         "adjoint_check": {"lhs": lhs, "rhs": rhs, "rel_diff": abs(lhs - rhs) / abs(lhs)},
     }

@@ -33,6 +33,22 @@ def test_circular_orbits_take_the_aligned_kernel(name, wmax):
         assert 16 <= max(ws) <= wmax, (name, max(ws))
 
 
+def test_wide_cones_take_the_tma_kernel_with_narrower_row_blocks():
+    """C5 / P1: the z window of 256 detector rows exceeds the largest TMA box (256 voxels); most poses fit with
+    192-row blocks and are planned FP_KERNEL_TMA with that window, the rest (C5 near 45 degrees: more than 12 volume
+    rows per slice) stay with the line-staging kernel and its wider window."""
+    for name, lo_frac in (("C5", 0.6), ("P1", 0.7)):
+        cfg = synth.CONFIGS[name]
+        geom = synth.make_geometry(cfg)
+        with fp.Projector(*cfg.n, cfg.voxel_size, cfg.origin) as P:
+            plans = [P.plan(geom[p], cfg.nu, cfg.nv) for p in range(0, cfg.n_proj, 4)]
+        tma = [w for k, w, z in plans if k == fp.KERNEL_TMA]
+        al = [w for k, w, z in plans if k == fp.KERNEL_ALIGNED]
+        assert len(tma) + len(al) == len(plans)
+        assert len(tma) >= lo_frac * len(plans) and len(al) > 0, (name, len(tma), len(al))
+        assert max(tma) <= 256 < min(al), (name, max(tma), min(al))
+
+
 def test_general_poses_take_the_tile_kernel_and_report_z_driven_rays():
     cfg = synth.CONFIGS["C4"]
     geom = synth.make_geometry(cfg)
