@@ -252,17 +252,36 @@ fp_bp_aligned_kernel(const __grid_constant__ BpParams P)
                         const bool a0 = (unsigned)k0 < nz, a1 = (unsigned)(k0 + 1) < nz;
                         const bool b0 = (unsigned)k1 < nz, b1 = (unsigned)(k1 + 1) < nz;
                         const bool r0 = tp.x != 0xFFFFFFFFu, r1 = tp.y != 0xFFFFFFFFu;
-                        float *qa = vol + ((long long)tp.x + k0), *qb = vol + ((long long)tp.x + k1);
-                        bp_red(qa, t00.x, r0 && a0);
-                        bp_red(qa + 1, t01m.x, r0 && a1);
-                        bp_red(qb, t00.y, r0 && b0);
-                        bp_red(qb + 1, t01m.y, r0 && b1);
-                        qa = vol + ((long long)tp.y + k0);
-                        qb = vol + ((long long)tp.y + k1);
-                        bp_red(qa, t10.x, r1 && a0);
-                        bp_red(qa + 1, t11m.x, r1 && a1);
-                        bp_red(qb, t10.y, r1 && b0);
-                        bp_red(qb + 1, t11m.y, r1 && b1);
+                        // one branch per detector row: a lane that dropped out in the merge (or whose row is past the
+                        // detector edge) skips its eight reductions together; the interior case runs them unguarded
+                        if (a0 || a1) {
+                            float *q0 = vol + ((long long)tp.x + k0), *q1 = vol + ((long long)tp.y + k0);
+                            if (a0 && a1 && r0 && r1) {
+                                atomicAdd(q0, t00.x);
+                                atomicAdd(q0 + 1, t01m.x);
+                                atomicAdd(q1, t10.x);
+                                atomicAdd(q1 + 1, t11m.x);
+                            } else {
+                                bp_red(q0, t00.x, r0 && a0);
+                                bp_red(q0 + 1, t01m.x, r0 && a1);
+                                bp_red(q1, t10.x, r1 && a0);
+                                bp_red(q1 + 1, t11m.x, r1 && a1);
+                            }
+                        }
+                        if (b0 || b1) {
+                            float *q0 = vol + ((long long)tp.x + k1), *q1 = vol + ((long long)tp.y + k1);
+                            if (b0 && b1 && r0 && r1) {
+                                atomicAdd(q0, t00.y);
+                                atomicAdd(q0 + 1, t01m.y);
+                                atomicAdd(q1, t10.y);
+                                atomicAdd(q1 + 1, t11m.y);
+                            } else {
+                                bp_red(q0, t00.y, r0 && b0);
+                                bp_red(q0 + 1, t01m.y, r0 && b1);
+                                bp_red(q1, t10.y, r1 && b0);
+                                bp_red(q1 + 1, t11m.y, r1 && b1);
+                            }
+                        }
                     }
                     // the plan of this stage has been read
                     __syncwarp();
