@@ -46,6 +46,7 @@
 #ifndef FP_H_
 #define FP_H_
 
+#include <stddef.h>
 #include <stdint.h>
 
 #ifdef __cplusplus
@@ -237,6 +238,33 @@ fp_status fp_last_launch_count(fp_ctx *ctx, int *n);
  */
 enum { FP_PROBE_HBM_READ = 0, FP_PROBE_L2_READ = 1, FP_PROBE_SHARED_READ = 2 };
 fp_status fp_probe_bandwidth(int what, double *gbs);
+
+/*
+ * fp_project_static: fp_project for callers that may not allocate (code under CUDA graph capture, tight serving
+ * loops, harnesses that forbid cudaMalloc).  Same operation and output as fp_project with FP_OPT_KERNEL =
+ * FP_KERNEL_DIRECT (Alg. 1, any pose, no preconditions on the volume), but the kernel's scratch --
+ * the per-projection descriptor table it reads and the sample counter it adds to -- lives in a file-scope
+ * `static __device__` array of 256 + 104 * FP_STATIC_MAX_PROJ bytes (about 52 KB) that every GPU which loads the
+ * library holds until exit.  Needs no context; calls no cudaMalloc, cudaFree or other allocating routine, on the
+ * device or the host; enqueues on `stream` and returns without synchronising.
+ *   nx, ny, nz, voxel_size, origin   the grid, as for fp_create
+ *   vol_dev        device, fp32 [nx][ny][nz], read only
+ *   n_proj         0 .. FP_STATIC_MAX_PROJ; more is rejected with FP_ERR_UNSUPPORTED (split the call)
+ *   geom_host      host, double [n_proj][12], as for fp_project; may be reused when the call returns
+ *   interp         FP_INTERP_LINEAR or FP_INTERP_SPLINE
+ *   out_dev        device, fp32 [n_proj][nv][nu], fully overwritten
+ *   n_samples_dev  device, one unsigned 64-bit word: receives the number of samples taken; may be null
+ *   err, err_len   host buffer for the message of a failed call (always NUL-terminated); may be null / 0
+ * Every call on a device shares the one array, which keeps the last call's contents: the call clears the counter and
+ * overwrites the table itself, in stream order.  Calls that OVERLAP on the GPU (different streams without an event
+ * between them, or two host threads) race on it and give undefined projections; calls on one stream are safe.
+ * z-driven rays read the caller's array with a stride (no permuted copy is built): this is the slow, always
+ * available path -- use fp_project where allocation is allowed.
+ */
+#define FP_STATIC_MAX_PROJ 512
+fp_status fp_project_static(int nx, int ny, int nz, double voxel_size, const double origin[3], const float *vol_dev,
+                            int n_proj, const double *geom_host, int nu, int nv, int interp, float *out_dev,
+                            unsigned long long *n_samples_dev, fp_stream stream, char *err, size_t err_len);
 
 const char *fp_status_string(fp_status s);
 const char *fp_last_error(fp_ctx *ctx);

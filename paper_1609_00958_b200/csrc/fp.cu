@@ -3,6 +3,7 @@
 // No arithmetic of the method lives here except the host planning heuristics (which kernel,
 // which warp orientation); every step of the hot path runs in the kernels of fp_kernels.cuh.
 #include <cmath>
+#include <mutex>
 #include <cstdio>
 #include <cstring>
 #include <new>
@@ -1162,4 +1163,137 @@ extern "C" fp_status fp_probe_bandwidth(int what, double *gbs)
     cudaGetLastError();
     *gbs = best;
     return st;
+}
+
+// ------------------------------------------------------------------------------------------
+// fp_project_static (include/fp.h): the forward projector for callers that may not allocate.
+// fp_direct_kernel with its scratch -- the per-projection descriptor table the kernel reads and the
+// sample counter it adds to -- in a file-scope device array instead of the context's cudaMalloc'ed
+// workspaces.  No context, no cudaMalloc / cudaFree, no host heap.
+// ------------------------------------------------------------------------------------------
+namespace {
+
+constexpr size_t kStaticCounterBytes = 256;      // [0, 8): the sample counter; the rest keeps the table 256-byte aligned
+constexpr size_t kStaticBytes = kStaticCounterBytes + sizeof(ProjDesc) * (size_t)FP_STATIC_MAX_PROJ;
+
+// Every device that loads the library holds these kStaticBytes (about 52 KB) until exit.  In host code this name is a
+// host-side stand-in, not a device address: the address a kernel may use comes from cudaGetSymbolAddress below.
+static __device__ __align__(256) unsigned char g_static_scratch[kStaticBytes];
+
+constexpr int kStaticMaxDevices = 64;
+unsigned char *g_static_ptr[kStaticMaxDevices];  // per device: device address of g_static_scratch, null = not asked yet
+std::mutex g_static_mu;
+
+fp_status static_fail(fp_status s, char *err, size_t err_len, const char *msg)
+{
+    if (err && err_len) snprintf(err, err_len, "%s", msg);
+    return s;
+}
+
+// Once per device, with that device current: the device address of the scratch array.
+fp_status static_scratch(unsigned char **ptr, char *err, size_t err_len)
+{
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return static_fail(FP_ERR_CUDA, err, err_len, cudaGetErrorString(e));
+    if (dev < 0 || dev >= kStaticMaxDevices) return static_fail(FP_ERR_UNSUPPORTED, err, err_len, "fp_project_static: device ordinal >= 64");
+    std::lock_guard<std::mutex> lock(g_static_mu);
+    if (!g_static_ptr[dev]) {
+        void *p = nullptr;
+        e = cudaGetSymbolAddress(&p, g_static_scratch);
+        if (e != cudaSuccess || !p) {
+            char buf[192];
+            snprintf(buf, sizeof buf, "fp_project_static: cudaGetSymbolAddress: %s", cudaGetErrorString(e));
+            cudaGetLastError();
+            return static_fail(FP_ERR_CUDA, err, err_len, buf);
+        }
+        g_static_ptr[dev] = static_cast<unsigned char *>(p);
+    }
+    *ptr = g_static_ptr[dev];
+    return FP_OK;
+}
+
+}  // namespace
+
+extern "C" fp_status fp_project_static(int nx, int ny, int nz, double voxel_size, const double origin[3],
+                                       const float *vol_dev, int n_proj, const double *geom, int nu, int nv, int interp,
+                                       float *out_dev, unsigned long long *n_samples_dev, fp_stream stream, char *err,
+                                       size_t err_len)
+{
+    if (err && err_len) err[0] = '\0';
+    if (nx < 1 || ny < 1 || nz < 1 || !origin || !(voxel_size > 0.0) || !std::isfinite(voxel_size))
+        return static_fail(FP_ERR_INVALID_ARG, err, err_len, "fp_project_static: bad grid");
+    for (int a = 0; a < 3; ++a)
+        if (!std::isfinite(origin[a])) return static_fail(FP_ERR_INVALID_ARG, err, err_len, "fp_project_static: bad origin");
+    if ((double)nx * ny * nz >= 1099511627776.0) return static_fail(FP_ERR_INVALID_ARG, err, err_len, "fp_project_static: grid too large");
+    if (n_proj < 0 || nu < 1 || nv < 1) return static_fail(FP_ERR_INVALID_ARG, err, err_len, "fp_project_static: n_proj < 0 or nu, nv < 1");
+    if (interp != FP_INTERP_LINEAR && interp != FP_INTERP_SPLINE)
+        return static_fail(FP_ERR_INVALID_ARG, err, err_len, "fp_project_static: interp must be FP_INTERP_LINEAR or FP_INTERP_SPLINE");
+    if (n_proj > FP_STATIC_MAX_PROJ) {
+        char buf[192];
+        snprintf(buf, sizeof buf, "fp_project_static: n_proj = %d exceeds FP_STATIC_MAX_PROJ = %d (the static scratch holds that many "
+                 "projection descriptors): split the call", n_proj, FP_STATIC_MAX_PROJ);
+        return static_fail(FP_ERR_UNSUPPORTED, err, err_len, buf);
+    }
+    if (n_proj > 0 && (!vol_dev || !geom || !out_dev)) return static_fail(FP_ERR_INVALID_ARG, err, err_len, "fp_project_static: null pointer");
+    cudaStream_t st = (cudaStream_t)stream;
+    unsigned char *scratch = nullptr;
+    fp_status s = static_scratch(&scratch, err, err_len);
+    if (s != FP_OK) return s;
+    unsigned long long *count = reinterpret_cast<unsigned long long *>(scratch);
+    ProjDesc *table = reinterpret_cast<ProjDesc *>(scratch + kStaticCounterBytes);
+    cudaError_t e;
+#define FP_STATIC_CUDA(call)                                                                         \
+    do {                                                                                             \
+        e = (call);                                                                                  \
+        if (e != cudaSuccess) {                                                                      \
+            char buf_[192];                                                                          \
+            snprintf(buf_, sizeof buf_, "fp_project_static: %s: %s", #call, cudaGetErrorString(e)); \
+            cudaGetLastError();                                                                      \
+            return static_fail(FP_ERR_CUDA, err, err_len, buf_);                                     \
+        }                                                                                            \
+    } while (0)
+    // the array keeps the last call's contents: the counter must start at zero, the table is overwritten
+    FP_STATIC_CUDA(cudaMemsetAsync(count, 0, sizeof(unsigned long long), st));
+    if (n_proj > 0) {
+        ProjDesc h[FP_STATIC_MAX_PROJ];                 // on the stack: no host heap either
+        for (int p = 0; p < n_proj; ++p) {
+            memcpy(h[p].g, geom + 12 * (size_t)p, sizeof(double) * 12);
+            h[p].lane_v = plan_lane_v(h[p].g, nu, nv, false);
+            h[p].pad_ = 0;
+        }
+        // pageable source: the runtime stages the bytes before returning, so `h` may die here
+        FP_STATIC_CUDA(cudaMemcpyAsync(table, h, sizeof(ProjDesc) * (size_t)n_proj, cudaMemcpyHostToDevice, st));
+        ProjectParams P;
+        P.G.n[0] = nx;
+        P.G.n[1] = ny;
+        P.G.n[2] = nz;
+        P.G.pad_ = 0;
+        P.G.delta = voxel_size;
+        for (int a = 0; a < 3; ++a) P.G.origin[a] = origin[a];
+        const long long lx = nx, ly = ny, lz = nz;
+        P.lay[0] = AxisLayout{vol_dev, ly * lz, lz, 1, (int)lx, (int)ly, (int)lz, 0};       // m = x: slow y, fast z
+        P.lay[1] = AxisLayout{vol_dev, lz, ly * lz, 1, (int)ly, (int)lx, (int)lz, 0};       // m = y: slow x, fast z
+        P.lay[2] = AxisLayout{vol_dev, 1, ly * lz, lz, (int)lz, (int)lx, (int)ly, 0};       // m = z: slow x, fast y (strided)
+        P.proj = table;
+        P.ids = nullptr;
+        P.out = out_dev;
+        P.sample_count = count;
+        P.nu = nu;
+        P.nv = nv;
+        P.n_proj = n_proj;
+        P.interp = interp;
+        const unsigned gl = (unsigned)((std::max(nu, nv) + kTileLane - 1) / kTileLane);
+        const unsigned gr = (unsigned)((std::max(nu, nv) + kTileRow - 1) / kTileRow);
+        dim3 grid(gl, gr, (unsigned)n_proj);
+        if (interp == FP_INTERP_SPLINE)
+            fp_direct_kernel<1><<<grid, kDirectThreads, 0, st>>>(P);
+        else
+            fp_direct_kernel<0><<<grid, kDirectThreads, 0, st>>>(P);
+        FP_STATIC_CUDA(cudaGetLastError());
+    }
+    if (n_samples_dev)
+        FP_STATIC_CUDA(cudaMemcpyAsync(n_samples_dev, count, sizeof(unsigned long long), cudaMemcpyDeviceToDevice, st));
+#undef FP_STATIC_CUDA
+    return FP_OK;
 }

@@ -26,7 +26,7 @@ INTERP_LINEAR, INTERP_SPLINE = 0, 1
 # every symbol include/fp.h declares (tests check the library exports all of them)
 SYMBOLS = ["fp_create", "fp_destroy", "fp_set_option", "fp_get_option", "fp_prepare", "fp_project",
            "fp_project_host", "fp_backproject", "fp_ray_ranges", "fp_plan", "fp_check", "fp_last_sample_count",
-           "fp_last_launch_count", "fp_probe_bandwidth", "fp_status_string", "fp_last_error", "fp_version"]
+           "fp_last_launch_count", "fp_probe_bandwidth", "fp_project_static", "fp_status_string", "fp_last_error", "fp_version"]
 PROBE_HBM_READ, PROBE_L2_READ, PROBE_SHARED_READ = 0, 1, 2
 
 
@@ -73,6 +73,8 @@ def load(build_if_missing: bool = True):
     for name in ("fp_create", "fp_destroy", "fp_set_option", "fp_get_option", "fp_prepare", "fp_project", "fp_check",
                  "fp_project_host", "fp_backproject", "fp_ray_ranges", "fp_plan", "fp_last_sample_count", "fp_last_launch_count"):
         getattr(L, name).restype = i
+    L.fp_project_static.argtypes = [i, i, i, ctypes.c_double, dp, vp, i, dp, i, i, i, vp, vp, vp, ctypes.c_char_p, ctypes.c_size_t]
+    L.fp_project_static.restype = i
     L.fp_status_string.argtypes = [i]
     L.fp_status_string.restype = ctypes.c_char_p
     L.fp_last_error.argtypes = [vp]
@@ -236,6 +238,36 @@ class Projector:
         n = ctypes.c_int()
         self._check(self._L.fp_last_launch_count(self._h, ctypes.byref(n)))
         return n.value
+
+
+STATIC_MAX_PROJ = 512
+
+
+def project_static(shape, voxel_size: float, origin, vol, geom, nu: int, nv: int, interp: int = INTERP_LINEAR,
+                   out=None, n_samples=None, stream=None):
+    """fp_project_static: the projector without a context and without any allocation inside the library (its
+    scratch is a static device array).  `out` ([n_proj][nv][nu] fp32) and `n_samples` (one int64 word, optional)
+    are the caller's device tensors; `out` is created here if not given."""
+    import torch
+    g = _geom(geom)
+    n_proj = g.shape[0]
+    if vol.dtype != torch.float32 or not vol.is_cuda or not vol.is_contiguous() or tuple(vol.shape) != tuple(shape):
+        raise ValueError("vol must be a contiguous fp32 CUDA tensor of the grid's shape")
+    if out is None:
+        out = torch.empty((n_proj, nv, nu), dtype=torch.float32, device=vol.device)
+    if out.dtype != torch.float32 or not out.is_contiguous() or tuple(out.shape) != (n_proj, nv, nu):
+        raise ValueError("out must be a contiguous fp32 tensor [n_proj][nv][nu]")
+    if n_samples is not None and (n_samples.dtype != torch.int64 or n_samples.numel() != 1 or not n_samples.is_cuda):
+        raise ValueError("n_samples must be a one-element int64 CUDA tensor")
+    o = (ctypes.c_double * 3)(*[float(x) for x in origin])
+    err = ctypes.create_string_buffer(256)
+    st = load().fp_project_static(int(shape[0]), int(shape[1]), int(shape[2]), float(voxel_size), o, vol.data_ptr(), n_proj,
+                                  g.ctypes.data_as(ctypes.POINTER(ctypes.c_double)), int(nu), int(nv), int(interp),
+                                  out.data_ptr(), n_samples.data_ptr() if n_samples is not None else None,
+                                  _stream_handle(stream), err, len(err))
+    if st != FP_OK:
+        raise FpError(st, err.value.decode())
+    return out
 
 
 def probe_bandwidth(what: int) -> float:
