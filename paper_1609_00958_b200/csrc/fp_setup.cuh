@@ -127,14 +127,15 @@ __device__ __forceinline__ int axis_slow(int m) { return m == 0 ? 1 : 0; }
 __device__ __forceinline__ int axis_fast(int m) { return m == 2 ? 1 : 2; }
 
 // g = { S xyz, O xyz, U xyz, V xyz } in world units; pixel centre D = (O + iu U) + iv V.
-__device__ __forceinline__ RaySetup ray_setup(const double *__restrict__ g, const GridDesc &G, int iu, int iv)
+// s = the source in grid units, (g[a] - origin[a]) / delta per axis in exactly these operations: the same for every
+// ray of a pose, so a block may compute it once (ray_setup below computes it per call).
+__device__ __forceinline__ RaySetup ray_setup_from(const double *__restrict__ g, const GridDesc &G, const double s[3], int iu, int iv)
 {
-    double s[3], r[3];
+    double r[3];
 #pragma unroll
     for (int a = 0; a < 3; ++a) {
         const double D = __dadd_rn(__dadd_rn(g[3 + a], __dmul_rn((double)iu, g[6 + a])),
                                    __dmul_rn((double)iv, g[9 + a]));
-        s[a] = __ddiv_rn(__dsub_rn(g[a], G.origin[a]), G.delta);
         const double d = __ddiv_rn(__dsub_rn(D, G.origin[a]), G.delta);
         r[a] = __dsub_rn(d, s[a]);                                   // Eq. 1
     }
@@ -167,6 +168,14 @@ __device__ __forceinline__ RaySetup ray_setup(const double *__restrict__ g, cons
     if (lo <= hi) clip_axis(R.s_b, R.s_m, R.rt_b, sel3i(tb, G.n[0], G.n[1], G.n[2]), lo, hi);
     if (lo <= hi) { R.i_first = lo; R.i_last = hi; }
     return R;
+}
+
+__device__ __forceinline__ RaySetup ray_setup(const double *__restrict__ g, const GridDesc &G, int iu, int iv)
+{
+    double s[3];
+#pragma unroll
+    for (int a = 0; a < 3; ++a) s[a] = __ddiv_rn(__dsub_rn(g[a], G.origin[a]), G.delta);
+    return ray_setup_from(g, G, s, iu, iv);
 }
 
 }  // namespace fpk

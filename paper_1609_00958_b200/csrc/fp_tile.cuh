@@ -217,8 +217,9 @@ fp_tile_kernel(const __grid_constant__ TileParams P)
     float scA = 0.0f, scB = 0.0f;
     double2 *rayp = reinterpret_cast<double2 *>(tl_smem_raw + kTlTileBytes + sizeof(TlShared));
     if (!producer) {
-        const RaySetup RA = ray_setup(g, P.G, min(iuA, P.nu - 1), min(ivA, P.nv - 1));
-        const RaySetup RB = ray_setup(g, P.G, min(iuB, P.nu - 1), min(ivB, P.nv - 1));
+        const double src[3] = {S.cs[0], S.cs[1], S.cs[2]};       // the source in grid units, computed once per block
+        const RaySetup RA = ray_setup_from(g, P.G, src, min(iuA, P.nu - 1), min(ivA, P.nv - 1));
+        const RaySetup RB = ray_setup_from(g, P.G, src, min(iuB, P.nu - 1), min(ivB, P.nv - 1));
         if (RA.i_last >= RA.i_first) { mA = RA.m; scA = (float)(P.G.delta * RA.L); }
         if (RB.i_last >= RB.i_first) { mB = RB.m; scB = (float)(P.G.delta * RB.L); }
         rayp[0 * kTlRaySlots + tid] = make_double2(RA.s_a, RA.rt_a);
