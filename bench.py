@@ -13,6 +13,7 @@ The oracle (oracle/) is used only by the cpu_baseline leg and by --impl referenc
 from __future__ import annotations
 
 import argparse
+import datetime
 import json
 import math
 import os
@@ -68,11 +69,14 @@ def measured_peaks():
 class ClockSampler:
     """nvidia-smi clocks and throttle reasons DURING the timed region (B200_PROFILING.md)."""
 
-    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,"
+    Q = ("timestamp,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,"
          "clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
          "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
 
     def __init__(self, gpu_index: int):
+        # started BEFORE the warm-up steps so that no idle gap (in which the clocks fall back) separates the
+        # warm-up from the timed region; only the samples stamped inside [mark_start, mark_end] are reported
+        self.t0 = self.t1 = None
         self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
         self.p = None
         try:
@@ -81,6 +85,22 @@ class ClockSampler:
                                       stdout=self.f, stderr=subprocess.DEVNULL)
         except Exception:
             self.p = None
+
+    def mark_start(self):
+        self.t0 = datetime.datetime.now()
+
+    def mark_end(self):
+        self.t1 = datetime.datetime.now()
+
+    def _inside(self, stamp: str) -> bool:
+        if self.t0 is None or self.t1 is None:
+            return True
+        try:
+            t = datetime.datetime.strptime(stamp, "%Y/%m/%d %H:%M:%S.%f")
+        except ValueError:
+            return True
+        slack = datetime.timedelta(milliseconds=50)
+        return self.t0 - slack <= t <= self.t1 + slack
 
     def stop(self):
         out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
@@ -93,12 +113,15 @@ class ClockSampler:
             self.p.kill()
         self.f.flush()
         self.f.seek(0)
-        sm, mx, reasons = [], [], set()
         names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
-        for line in self.f.read().splitlines():
-            c = [x.strip() for x in line.split(",")]
-            if len(c) < 9:
-                continue
+        lines = [[x.strip() for x in line.split(",")] for line in self.f.read().splitlines()]
+        lines = [c for c in lines if len(c) >= 9]
+        inside = [c for c in lines if self._inside(c[0])]
+        # a timed region shorter than the sampling period (C1, C2) has no sample of its own: then the samples of
+        # the warm-up steps right before it stand in, and the line says so
+        out["window"] = "timed region" if inside else "whole run (timed region shorter than the sampling period)"
+        sm, mx, reasons = [], [], set()
+        for c in (inside or lines):
             try:
                 sm.append(float(c[1]))
                 mx.append(float(c[2]))
@@ -212,18 +235,19 @@ def run_backproject(args, torch, fp, cfg, geom, vol, proj, P, stream, world, ran
         P.backproject(proj, geom, cfg.nu, cfg.nv, out=bp, stream=stream)
         return P.last_launch_count()
 
+    clocks = ClockSampler(int(os.environ.get("LOCAL_RANK", "0")))
     for _ in range(args.warmup):
         step()
     torch.cuda.synchronize()
     ev = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps + 1)]
-    clocks = ClockSampler(int(os.environ.get("LOCAL_RANK", "0")))
-    time.sleep(0.25)
     launches = 0
+    clocks.mark_start()
     ev[0].record(stream)
     for k in range(args.steps):
         launches += step()
         ev[k + 1].record(stream)
     torch.cuda.synchronize()
+    clocks.mark_end()
     clk = clocks.stop()
     ms = max_over_ranks(dist, ev[0].elapsed_time(ev[args.steps])) / args.steps
     if rank != 0:
@@ -342,6 +366,7 @@ def main():
     # sample count of one step (outside the timed region: fp_last_sample_count synchronises, and the
     # count costs one exact fp64 ray set-up per ray that the sampling itself does not need)
     samples = 0
+    clocks = ClockSampler(local_rank)
     P.set_option(fp.OPT_COUNT_SAMPLES, 1)
     for p0 in range(0, cfg.n_proj, batch):
         p1 = min(cfg.n_proj, p0 + batch)
@@ -355,14 +380,14 @@ def main():
     ev = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps + 1)]
     barrier()
     torch.cuda.synchronize()
-    clocks = ClockSampler(local_rank)
-    time.sleep(0.25)
     launches = 0
+    clocks.mark_start()
     ev[0].record(stream)
     for k in range(args.steps):
         launches += step()
         ev[k + 1].record(stream)
     torch.cuda.synchronize()
+    clocks.mark_end()
     barrier()
     clk = clocks.stop()
     P.check()                                    # no kernel found the host plan too small

@@ -71,9 +71,13 @@ __device__ __forceinline__ void clip_axis(double s_t, double s_m, double rt_t, i
         if (!((-1.0 < p) && (p < nt))) hi = lo - 1;
         return;
     }
-    // real-valued slice positions where p_t = -1 and p_t = N_t
-    const double x_m1 = __dadd_rn(s_m, __ddiv_rn(__dsub_rn(-1.0, s_t), rt_t));
-    const double x_nt = __dadd_rn(s_m, __ddiv_rn(__dsub_rn(nt, s_t), rt_t));
+    // real-valued slice positions where p_t = -1 and p_t = N_t.  They are ESTIMATES only -- the fix-up below
+    // evaluates the defining predicate and ends on its exact extreme slice whatever the estimate was -- so an fp32
+    // reciprocal (|rt_t| <= 1: no overflow; a denormal rt_t gives inf / NaN, which clamp_to_int absorbs) replaces
+    // the two fp64 divisions: four of the ten divisions of a ray's set-up
+    const double inv = (double)__frcp_rn((float)rt_t);
+    const double x_m1 = __dadd_rn(s_m, __dmul_rn(__dsub_rn(-1.0, s_t), inv));
+    const double x_nt = __dadd_rn(s_m, __dmul_rn(__dsub_rn(nt, s_t), inv));
     const bool up = rt_t > 0.0;
     // "enter": inequality false -> true with growing i; "leave": true -> false
     const double x_enter = up ? x_m1 : x_nt;
@@ -129,14 +133,34 @@ __device__ __forceinline__ int axis_fast(int m) { return m == 2 ? 1 : 2; }
 // g = { S xyz, O xyz, U xyz, V xyz } in world units; pixel centre D = (O + iu U) + iv V.
 // s = the source in grid units, (g[a] - origin[a]) / delta per axis in exactly these operations: the same for every
 // ray of a pose, so a block may compute it once (ray_setup below computes it per call).
+// x / delta (Eq. 1's world -> grid map).  Where delta is a power of two -- every BASELINE configuration -- the
+// product with the exactly representable 1 / delta is the same correctly rounded value as the quotient (the two
+// real numbers are equal), so the division is skipped; the test is uniform over the launch.
+struct GridScale {
+    double inv;          // 1 / delta if delta is a power of two with a representable reciprocal, else 0
+};
+__device__ __forceinline__ GridScale grid_scale(double delta)
+{
+    const long long b = __double_as_longlong(delta);
+    const long long e = (b >> 52) & 0x7ffLL;
+    GridScale K;
+    K.inv = (b > 0 && (b & 0x000fffffffffffffLL) == 0 && e >= 2 && e <= 2044) ? __longlong_as_double((2046LL - e) << 52) : 0.0;
+    return K;
+}
+__device__ __forceinline__ double to_grid(double x, double delta, const GridScale &K)
+{
+    return K.inv != 0.0 ? __dmul_rn(x, K.inv) : __ddiv_rn(x, delta);
+}
+
 __device__ __forceinline__ RaySetup ray_setup_from(const double *__restrict__ g, const GridDesc &G, const double s[3], int iu, int iv)
 {
+    const GridScale K = grid_scale(G.delta);
     double r[3];
 #pragma unroll
     for (int a = 0; a < 3; ++a) {
         const double D = __dadd_rn(__dadd_rn(g[3 + a], __dmul_rn((double)iu, g[6 + a])),
                                    __dmul_rn((double)iv, g[9 + a]));
-        const double d = __ddiv_rn(__dsub_rn(D, G.origin[a]), G.delta);
+        const double d = to_grid(__dsub_rn(D, G.origin[a]), G.delta, K);
         r[a] = __dsub_rn(d, s[a]);                                   // Eq. 1
     }
     RaySetup R;
@@ -151,18 +175,19 @@ __device__ __forceinline__ RaySetup ray_setup_from(const double *__restrict__ g,
     double rm = r[0];
     if (fabs(r[1]) > fabs(rm)) { m = 1; rm = r[1]; }
     if (fabs(r[2]) > fabs(rm)) { m = 2; rm = r[2]; }
-    double rt0 = __ddiv_rn(r[0], rm), rt1 = __ddiv_rn(r[1], rm), rt2 = __ddiv_rn(r[2], rm);  // Eq. 4
-    if (m == 0) rt0 = 1.0;
-    if (m == 1) rt1 = 1.0;
-    if (m == 2) rt2 = 1.0;
-    R.L = sqrt(__dadd_rn(__dadd_rn(__dmul_rn(rt0, rt0), __dmul_rn(rt1, rt1)), __dmul_rn(rt2, rt2)));
     const int ta = axis_slow(m), tb = axis_fast(m);
+    // Eq. 4: two divisions, r~_m := 1 (reading #9)
+    const double rta = __ddiv_rn(sel3(ta, r[0], r[1], r[2]), rm), rtb = __ddiv_rn(sel3(tb, r[0], r[1], r[2]), rm);
+    const double rt0 = m == 0 ? 1.0 : rta;                           // ta = x unless m = x
+    const double rt1 = m == 1 ? 1.0 : (m == 0 ? rta : rtb);          // y is the slow axis for m = x, the fast one for m = z
+    const double rt2 = m == 2 ? 1.0 : rtb;                           // tb = z unless m = z
+    R.L = sqrt(__dadd_rn(__dadd_rn(__dmul_rn(rt0, rt0), __dmul_rn(rt1, rt1)), __dmul_rn(rt2, rt2)));
     R.m = m;
     R.s_m = sel3(m, s[0], s[1], s[2]);
     R.s_a = sel3(ta, s[0], s[1], s[2]);
     R.s_b = sel3(tb, s[0], s[1], s[2]);
-    R.rt_a = sel3(ta, rt0, rt1, rt2);
-    R.rt_b = sel3(tb, rt0, rt1, rt2);
+    R.rt_a = rta;
+    R.rt_b = rtb;
     int lo = 0, hi = sel3i(m, G.n[0], G.n[1], G.n[2]) - 1;
     clip_axis(R.s_a, R.s_m, R.rt_a, sel3i(ta, G.n[0], G.n[1], G.n[2]), lo, hi);
     if (lo <= hi) clip_axis(R.s_b, R.s_m, R.rt_b, sel3i(tb, G.n[0], G.n[1], G.n[2]), lo, hi);

@@ -319,6 +319,62 @@ def test_reuse_context_changed_volume_and_streams(torch, fp, synth, oracle):
             assert assert_parity(out.cpu().numpy().ravel(), gm.reshape(-1, 3), ov, om, pl, mg, float(np.abs(v).max())) < 1.0
 
 
+def test_host_plan_is_reused_only_for_the_same_geometry_and_options(torch, fp, synth):
+    """fp_project keeps the host plan of its last call (libfp's PlanCache, fp.cu) and reuses it when the next call
+    brings the same geometry, detector, options and volume alignment.  One context is driven through aligned poses,
+    general poses of the same count, the aligned poses again (a hit), then the same poses with another kernel
+    option (must re-plan): every result equals the one a fresh context gives, bit for bit."""
+    cfg = synth.CONFIGS["C2"]
+    vol = synth.make_volume(cfg, device="cuda")
+    nu = nv = 96
+    g_al = synth.make_geometry(cfg)[[0, 44, 45, 46, 90, 133]].copy()
+    for g in g_al:                                    # same orbit, smaller detector: keep it centred
+        g[3:6] += (cfg.nu - nu) / 2 * g[6:9] + (cfg.nv - nv) / 2 * g[9:12]
+    g_ge = synth.make_geometry(synth.CONFIGS["C4"])[:6].copy()
+    g_ge[:, :6] *= 128.0 / 512.0                      # C4's general poses, scaled to the 128^3 grid
+    g_ge[:, 6:] *= 3.0
+
+    def fresh(geom, options=()):
+        with fp.Projector(*cfg.n, cfg.voxel_size, cfg.origin) as Q:
+            for k, v in options:
+                Q.set_option(k, v)
+            o = Q.project(vol, geom, nu, nv)
+            torch.cuda.synchronize()
+            return o.cpu().numpy()
+
+    ref_al, ref_ge = fresh(g_al), fresh(g_ge)
+    ref_di = fresh(g_al, [(fp.OPT_KERNEL, fp.KERNEL_DIRECT)])
+    assert np.abs(ref_al).max() > 0 and np.abs(ref_ge).max() > 0
+    with fp.Projector(*cfg.n, cfg.voxel_size, cfg.origin) as P:
+        seq = [(g_al, ref_al), (g_al, ref_al), (g_ge, ref_ge), (g_al, ref_al), (g_ge, ref_ge), (g_ge, ref_ge)]
+        for k, (g, ref) in enumerate(seq):
+            o = P.project(vol, g, nu, nv)
+            torch.cuda.synchronize()
+            assert np.array_equal(o.cpu().numpy(), ref), "call %d" % k
+        P.check()
+        P.set_option(fp.OPT_KERNEL, fp.KERNEL_DIRECT)  # same geometry as the last aligned call, other plan
+        for g, ref in ((g_al, ref_di), (g_al, ref_di)):
+            o = P.project(vol, g, nu, nv)
+            torch.cuda.synchronize()
+            assert np.array_equal(o.cpu().numpy(), ref)
+        P.set_option(fp.OPT_KERNEL, fp.KERNEL_AUTO)
+        o = P.project(vol, g_al, nu, nv)
+        torch.cuda.synchronize()
+        assert np.array_equal(o.cpu().numpy(), ref_al)
+        # a volume view that is only 4-byte aligned: the aligned-class kernels need 16 bytes, so the plan changes
+        flat = torch.zeros(vol.numel() + 4, device="cuda", dtype=torch.float32)
+        v1 = flat[1:1 + vol.numel()].view(vol.shape)
+        v1.copy_(vol)
+        o = P.project(v1, g_al, nu, nv)
+        torch.cuda.synchronize()
+        o = o.cpu().numpy()
+        P.check()
+        assert np.allclose(o, ref_al, rtol=1e-4, atol=1e-4 * float(np.abs(ref_al).max()))
+        o = P.project(vol, g_al, nu, nv)
+        torch.cuda.synchronize()
+        assert np.array_equal(o.cpu().numpy(), ref_al)
+
+
 # ----------------------------------------------------------------------------- aligned kernel edge cases
 
 def aligned_pose(theta, sid, sdd, nu, nv, pitch, src_z=0.0, det_shift=(0.0, 0.0), flip_u=False, flip_v=False):
