@@ -87,6 +87,11 @@ class ClockSampler:
             self.p = None
 
     def mark_start(self):
+        # nvidia-smi needs about 0.2 s to print its first sample: a run whose warm-up is shorter than that (C1, C2)
+        # waits for it here, so that at least that sample stands in for a timed region of a few milliseconds
+        t_end = time.time() + 1.0
+        while self.p is not None and os.path.getsize(self.f.name) == 0 and time.time() < t_end:
+            time.sleep(0.01)
         self.t0 = datetime.datetime.now()
 
     def mark_end(self):
