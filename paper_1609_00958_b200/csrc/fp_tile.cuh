@@ -199,15 +199,20 @@ fp_tile_kernel(const __grid_constant__ TileParams P)
     }
     int iuA = 0, ivA = 0, iuB = 0, ivB = 0;
     if (!producer) {
-        const int w = tid >> 5;
-        if (!lanes_v) {                                       // 32 lanes along u; rows w and w + 8
-            iuA = iuB = tu0 + lane;
-            ivA = tv0 + w;
-            ivB = tv0 + w + 8;
-        } else {                                              // 16 lanes along v; two neighbouring columns per thread
-            ivA = ivB = tv0 + (lane & 15);
-            iuA = tu0 + 2 * (2 * w + (lane >> 4));
-            iuB = iuA + 1;
+        // A warp's 32 rays of one tap load form a 4 x 8 pixel patch, 4 along the detector axis that maps onto the
+        // contiguous in-plane axis: about 3 x 7 voxels of the slice plane, 8 tile rows of 4 words each.  With the
+        // tile pitches of the box classes (28, 36, 44, 52, 68 words = 4, 12 or 20 modulo 32 up to sign) consecutive tile
+        // rows are 4 banks apart, so the patch's words fall into distinct banks: 1.3-1.5 shared-memory wavefronts
+        // per load where a line of 32 pixels, which crosses tile rows at a stride the pitch does not match, needs 2.1.
+        const int w = tid >> 5, la = lane & 3, lb = lane >> 2;
+        if (!lanes_v) {                                       // patch: 4 along u x 8 along v; rays A, B: the two halves in v
+            iuA = iuB = tu0 + 4 * w + la;
+            ivA = tv0 + lb;
+            ivB = tv0 + lb + 8;
+        } else {                                              // patch: 4 along v x 8 along u; rays A, B: neighbouring patches in u
+            ivA = ivB = tv0 + 4 * (w & 3) + la;
+            iuA = tu0 + 16 * (w >> 2) + lb;
+            iuB = iuA + 8;
         }
     }
     const bool liveA = !producer && iuA < P.nu && ivA < P.nv, liveB = !producer && iuB < P.nu && ivB < P.nv;
