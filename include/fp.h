@@ -152,6 +152,11 @@ fp_status fp_prepare(fp_ctx *ctx, const float *vol_dev, fp_stream stream);
  *   geom_host  host, double [n_proj][12]
  *   nu, nv     >= 1 detector pixels along u and v
  *   out_dev    device, fp32 [n_proj][nv][nu], fully overwritten
+ * geom_host is read before the call returns (the caller may reuse the array).  The context keeps the host plan of its
+ * most recent fp_project call -- which kernel takes which pose -- together with a copy of that call's geometry, and
+ * reuses the plan when the next call brings bit-identical geometry, the same nu, nv, kernel option and volume
+ * alignment (the calls of an iterative reconstruction); anything else re-plans.  The results do
+ * not depend on whether the plan was reused.
  */
 fp_status fp_project(fp_ctx *ctx, const float *vol_dev, int n_proj, const double *geom_host,
                      int nu, int nv, float *out_dev, fp_stream stream);
