@@ -353,25 +353,25 @@ fp_tile_kernel(const __grid_constant__ TileParams P)
                 // the first column on a 16-byte boundary of the volume's rows (the TMA engine traps otherwise)
                 const int o_t = co ? ((__double2int_rd(pmin) - 1) & ~3) : (__double2int_rd(pmin) - 1);
                 const int js0_l = __shfl_sync(0xffffffffu, o_t, 8 * sb), kf0_l = __shfl_sync(0xffffffffu, o_t, 8 * sb + 1);
+                // the part of the published origin that depends on the box position, once per batch on all lanes
+                const unsigned rel_l = (0x4B400000u + (unsigned)js0_l) * pitchB + ((0x4B400000u + (unsigned)kf0_l) << 2);
                 for (int q = 0; q < 4 && n0 + q < n_slices; ++q) {
                     const int n = n0 + q;
                     const int js0 = __shfl_sync(0xffffffffu, js0_l, 8 * q), kf0 = __shfl_sync(0xffffffffu, kf0_l, 8 * q);
+                    const unsigned rel = __shfl_sync(0xffffffffu, rel_l, 8 * q);
                     if (n >= nst) tm_mbar_wait(&S.empty[st], ph);
                     if (lane == 0) {
                         // the consumers' reads of this stage (generic proxy, ordered before this point by their
                         // arrival on empty[]) before the copy below (async proxy)
                         tm_fence_proxy_async();
                         // consumers add bits(row) * pitch + bits(col) * 4 with bits = 0x4B400000 + index (mod 2^32)
-                        S.org[st].x = tiles_smem + st * stageB - ((0x4B400000u + (unsigned)js0) * pitchB + ((0x4B400000u + (unsigned)kf0) << 2));
-                        tm_mbar_arrive_tx(&S.full[st], boxB);
                         const unsigned dst = tiles_smem + st * stageB;
+                        S.org[st].x = dst - rel;
+                        tm_mbar_arrive_tx(&S.full[st], boxB);
                         const int ii = lo + n;
                         // tensor dimensions, fastest first: m = x: (z, y, x); m = y: (z, y, x) with the slow axis x;
                         // m = z: the y-fastest copy (y, x, z)
-                        if (m == 1)
-                            tm_load_3d(map, dst, &S.full[st], kf0, ii, js0);
-                        else
-                            tm_load_3d(map, dst, &S.full[st], kf0, js0, ii);
+                        tm_load_3d(map, dst, &S.full[st], kf0, m == 1 ? ii : js0, m == 1 ? js0 : ii);
                     }
                     __syncwarp();
                     if (++st == nst) {
