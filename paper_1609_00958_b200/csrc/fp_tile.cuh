@@ -357,10 +357,12 @@ fp_tile_kernel(const __grid_constant__ TileParams P)
                 const unsigned rel_l = (0x4B400000u + (unsigned)js0_l) * pitchB + ((0x4B400000u + (unsigned)kf0_l) << 2);
                 for (int q = 0; q < 4 && n0 + q < n_slices; ++q) {
                     const int n = n0 + q;
-                    const int js0 = __shfl_sync(0xffffffffu, js0_l, 8 * q), kf0 = __shfl_sync(0xffffffffu, kf0_l, 8 * q);
-                    const unsigned rel = __shfl_sync(0xffffffffu, rel_l, 8 * q);
+                    // slice q of the batch is issued by the lane that already holds its box position (lane 8 q): no
+                    // broadcast of the position per slice
+                    const int js0 = js0_l, kf0 = kf0_l;
+                    const unsigned rel = rel_l;
                     if (n >= nst) tm_mbar_wait(&S.empty[st], ph);
-                    if (lane == 0) {
+                    if (lane == 8 * q) {
                         // the consumers' reads of this stage (generic proxy, ordered before this point by their
                         // arrival on empty[]) before the copy below (async proxy)
                         tm_fence_proxy_async();
