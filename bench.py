@@ -118,8 +118,20 @@ class ClockSampler:
             self.p.kill()
         self.f.flush()
         self.f.seek(0)
+        out = self.summarize(self.f.read())
+        self.f.close()
+        try:
+            os.unlink(self.f.name)
+        except OSError:
+            pass
+        return out
+
+    def summarize(self, text: str) -> dict:
+        """Median SM clock, maximum clock and throttle reasons of the nvidia-smi samples stamped inside
+        [mark_start, mark_end] (host logic, covered by tests/test_bench_host.py)."""
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
         names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
-        lines = [[x.strip() for x in line.split(",")] for line in self.f.read().splitlines()]
+        lines = [[x.strip() for x in line.split(",")] for line in text.splitlines()]
         lines = [c for c in lines if len(c) >= 9]
         inside = [c for c in lines if self._inside(c[0])]
         # a timed region shorter than the sampling period (C1, C2) has no sample of its own: then the samples of
@@ -135,11 +147,6 @@ class ClockSampler:
             for n, v in zip(names, c[5:9]):
                 if v.lower().startswith("active"):
                     reasons.add(n)
-        self.f.close()
-        try:
-            os.unlink(self.f.name)
-        except OSError:
-            pass
         if sm:
             out.update(sm_mhz=statistics.median(sm), sm_max_mhz=max(mx), samples=len(sm))
         out["reasons"] = sorted(reasons)
